@@ -1,0 +1,246 @@
+"""paper_2301_07331_b200 -- B200-native HLC2 cross-match hot path.
+
+Thin Python binding over ``libhlc2.so`` (the C ABI of ``include/hlc2.h``): the functions below
+have the same names as the C entry points and only marshal arguments.  Every step of the path
+(validation, cell keys, radix sort, gather, cell table, match, compaction) runs in the library's
+hand-written sm_100a kernels.  PyTorch is used for device memory and streams only.
+
+There is no CPU fallback: if the library has not been built (``python -m
+paper_2301_07331_b200.build``) or no CUDA device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from dataclasses import dataclass
+
+HLC2_ALL_PAIRS = 0
+HLC2_NEAREST = 1
+
+HLC2_OK = 0
+HLC2_ERR_INVALID_ARG = -1
+HLC2_ERR_RADIUS_TOO_LARGE = -2
+HLC2_ERR_BUFFER_TOO_SMALL = -3
+HLC2_ERR_BAD_COORD = -4
+HLC2_ERR_CUDA = -5
+HLC2_ERR_GRID_MISMATCH = -6
+HLC2_ERR_TOO_MANY = -7
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhlc2.so")
+_lib = None
+
+
+class Hlc2Error(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = lib().hlc2_strerror(status).decode()
+        if status == HLC2_ERR_CUDA:
+            s = ctypes.c_char_p()
+            code = lib().hlc2_last_cuda_error(ctypes.byref(s))
+            msg += f" [cuda {code}: {s.value.decode() if s.value else '?'}]"
+        super().__init__(f"{where}: {msg} ({status})")
+
+
+class hlc2_opts(ctypes.Structure):
+    _fields_ = [("r_max_arcsec", ctypes.c_double), ("target_occupancy", ctypes.c_double),
+                ("cell_arcsec", ctypes.c_double), ("full_sky", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("grid_like", ctypes.c_void_p)]
+
+
+class hlc2_grid_info(ctypes.Structure):
+    _fields_ = [("dec_lo_deg", ctypes.c_double), ("zone_height_deg", ctypes.c_double), ("n_zones", ctypes.c_int64),
+                ("ra0_deg", ctypes.c_double), ("ra_span_deg", ctypes.c_double), ("n_cells", ctypes.c_int64),
+                ("cell_arcsec", ctypes.c_double), ("n", ctypes.c_int64)]
+
+
+def lib():
+    """Load libhlc2.so; fail loudly if it is missing (no fallback path exists)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2301_07331_b200.build` "
+                              "(the CUDA library is the only implementation; there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, i64, sz = ctypes.c_void_p, ctypes.c_int64, ctypes.c_size_t
+        P = ctypes.POINTER
+        L.hlc2_index_sizes.argtypes = [i64, P(hlc2_opts), P(sz), P(sz)]
+        L.hlc2_build_index.argtypes = [vp, vp, vp, i64, P(hlc2_opts), vp, sz, vp, sz, vp, P(vp)]
+        L.hlc2_index_status.argtypes = [vp, P(i64)]
+        L.hlc2_grid_describe.argtypes = [vp, P(hlc2_grid_info), P(P(ctypes.c_int32))]
+        L.hlc2_index_arrays.argtypes = [vp] + [P(vp)] * 6 + [P(i64), P(i64)]
+        L.hlc2_crossmatch_sizes.argtypes = [vp, vp, P(sz)]
+        L.hlc2_crossmatch.argtypes = [vp, vp, ctypes.c_double, ctypes.c_int, vp, vp, vp, i64, vp, vp, sz, vp]
+        L.hlc2_stream_sizes.argtypes = [i64, i64, P(hlc2_opts), i64, P(sz)]
+        L.hlc2_stream_crossmatch.argtypes = [vp] * 8 + [vp, i64, ctypes.c_double, ctypes.c_int, P(hlc2_opts),
+                                                        vp, vp, vp, i64, vp, vp, sz, i64]
+        L.hlc2_index_destroy.argtypes = [vp]
+        L.hlc2_index_destroy.restype = None
+        L.hlc2_strerror.argtypes = [ctypes.c_int]
+        L.hlc2_strerror.restype = ctypes.c_char_p
+        L.hlc2_last_cuda_error.argtypes = [P(ctypes.c_char_p)]
+        L.hlc2_kernel_launches.restype = ctypes.c_ulonglong
+        L.hlc2_version.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2301_07331_b200 needs a CUDA device (B200, sm_100a); there is no CPU fallback")
+    return torch
+
+
+def _stream_ptr(stream):
+    torch = _torch()
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def make_opts(r_max_arcsec=1.0, target_occupancy=0.0, cell_arcsec=0.0, full_sky=False, grid_like=None) -> hlc2_opts:
+    o = hlc2_opts()
+    o.r_max_arcsec = float(r_max_arcsec); o.target_occupancy = float(target_occupancy)
+    o.cell_arcsec = float(cell_arcsec); o.full_sky = int(bool(full_sky)); o.reserved = 0
+    o.grid_like = grid_like.handle if grid_like is not None else None
+    return o
+
+
+@dataclass
+class Index:
+    """A built index: the opaque handle plus the torch buffer that owns its device memory."""
+    handle: ctypes.c_void_p
+    buf: object            # torch.uint8 CUDA tensor (the caller-owned d_index_buf)
+    n: int
+    opts: hlc2_opts
+    _like: object = None   # keeps a grid_like index alive
+
+    def __del__(self):
+        try:
+            if self.handle:
+                lib().hlc2_index_destroy(self.handle)
+                self.handle = None
+        except Exception:
+            pass
+
+
+def hlc2_index_sizes(n: int, opts: hlc2_opts | None = None):
+    ib, tb = ctypes.c_size_t(0), ctypes.c_size_t(0)
+    rc = lib().hlc2_index_sizes(int(n), ctypes.byref(opts) if opts is not None else None, ctypes.byref(ib), ctypes.byref(tb))
+    if rc != HLC2_OK:
+        raise Hlc2Error(rc, "hlc2_index_sizes")
+    return ib.value, tb.value
+
+
+def hlc2_build_index(ra_deg, dec_deg, ids=None, opts: hlc2_opts | None = None, stream=None, temp=None,
+                     like: Index | None = None) -> Index:
+    """ra_deg, dec_deg: CUDA float64 tensors [n]; ids: CUDA int64 tensor [n] or None (row numbers)."""
+    torch = _torch()
+    n = int(ra_deg.shape[0])
+    if opts is None:
+        opts = make_opts()
+    if like is not None:
+        opts.grid_like = like.handle
+    assert ra_deg.is_cuda and dec_deg.is_cuda and ra_deg.dtype == torch.float64 and dec_deg.dtype == torch.float64
+    assert ra_deg.is_contiguous() and dec_deg.is_contiguous() and dec_deg.shape[0] == n
+    if ids is not None:
+        assert ids.is_cuda and ids.dtype == torch.int64 and ids.is_contiguous() and ids.shape[0] == n
+    ib, tb = hlc2_index_sizes(n, opts)
+    buf = torch.empty(ib, dtype=torch.uint8, device=ra_deg.device)
+    if temp is None or temp.numel() < tb:
+        temp = torch.empty(tb, dtype=torch.uint8, device=ra_deg.device)
+    out = ctypes.c_void_p()
+    rc = lib().hlc2_build_index(ra_deg.data_ptr(), dec_deg.data_ptr(), ids.data_ptr() if ids is not None else None,
+                                n, ctypes.byref(opts), buf.data_ptr(), ib, temp.data_ptr(), temp.numel(),
+                                _stream_ptr(stream), ctypes.byref(out))
+    if rc != HLC2_OK:
+        raise Hlc2Error(rc, "hlc2_build_index")
+    # the stream still owns `temp` until the enqueued work drains
+    temp.record_stream(torch.cuda.current_stream() if stream is None else stream)
+    return Index(out, buf, n, opts, like)
+
+
+def hlc2_index_status(idx: Index):
+    row = ctypes.c_int64(-1)
+    rc = lib().hlc2_index_status(idx.handle, ctypes.byref(row))
+    if rc not in (HLC2_OK, HLC2_ERR_BAD_COORD):
+        raise Hlc2Error(rc, "hlc2_index_status")
+    return rc, row.value
+
+
+def hlc2_grid_describe(idx: Index) -> dict:
+    import numpy as np
+    info = hlc2_grid_info()
+    p = ctypes.POINTER(ctypes.c_int32)()
+    rc = lib().hlc2_grid_describe(idx.handle, ctypes.byref(info), ctypes.byref(p))
+    if rc != HLC2_OK:
+        raise Hlc2Error(rc, "hlc2_grid_describe")
+    n_ra = np.ctypeslib.as_array(p, shape=(info.n_zones,)).copy()
+    return dict(dec_lo=info.dec_lo_deg, zone_h=info.zone_height_deg, n_zones=int(info.n_zones), ra0=info.ra0_deg,
+                span=info.ra_span_deg, n_cells=int(info.n_cells), cell_arcsec=info.cell_arcsec, n=int(info.n), n_ra=n_ra)
+
+
+def hlc2_index_arrays(idx: Index) -> dict:
+    """Torch views (no copies) of the index's device arrays."""
+    torch = _torch()
+    ptrs = [ctypes.c_void_p() for _ in range(6)]
+    n, nc = ctypes.c_int64(0), ctypes.c_int64(0)
+    rc = lib().hlc2_index_arrays(idx.handle, *[ctypes.byref(p) for p in ptrs], ctypes.byref(n), ctypes.byref(nc))
+    if rc != HLC2_OK:
+        raise Hlc2Error(rc, "hlc2_index_arrays")
+    base = idx.buf.data_ptr()
+
+    def view(p, count, dtype, size):
+        off = p.value - base
+        return idx.buf[off: off + count * size].view(dtype)
+
+    return dict(x=view(ptrs[0], n.value, torch.float64, 8), y=view(ptrs[1], n.value, torch.float64, 8),
+                z=view(ptrs[2], n.value, torch.float64, 8), id=view(ptrs[3], n.value, torch.int64, 8),
+                cell_start=view(ptrs[4], nc.value + 1, torch.int32, 4), cell_key=view(ptrs[5], n.value, torch.int32, 4),
+                n=n.value, n_cells=nc.value)
+
+
+def hlc2_crossmatch_sizes(A: Index, B: Index) -> int:
+    tb = ctypes.c_size_t(0)
+    rc = lib().hlc2_crossmatch_sizes(A.handle, B.handle, ctypes.byref(tb))
+    if rc != HLC2_OK:
+        raise Hlc2Error(rc, "hlc2_crossmatch_sizes")
+    return tb.value
+
+
+def hlc2_crossmatch(A: Index, B: Index, radius_arcsec: float, mode: int, out_ida, out_idb, out_sep, count,
+                    stream=None, temp=None):
+    """Raw call: out_* are CUDA tensors of `capacity` rows, `count` a CUDA tensor of one uint64/int64.
+    Asynchronous on `stream`; read `count` after synchronising."""
+    cap = int(out_ida.shape[0])
+    assert out_idb.shape[0] == cap and out_sep.shape[0] == cap
+    rc = lib().hlc2_crossmatch(A.handle, B.handle, float(radius_arcsec), int(mode), out_ida.data_ptr(), out_idb.data_ptr(),
+                               out_sep.data_ptr(), cap, count.data_ptr(), temp.data_ptr() if temp is not None else None,
+                               temp.numel() if temp is not None else 0, _stream_ptr(stream))
+    if rc != HLC2_OK:
+        raise Hlc2Error(rc, "hlc2_crossmatch")
+
+
+def crossmatch(A: Index, B: Index, radius_arcsec: float, mode: int = HLC2_ALL_PAIRS, capacity: int | None = None):
+    """Convenience: allocate outputs, call hlc2_crossmatch, retry once with the exact size if the first
+    buffer was too small.  Returns CUDA tensors (idA, idB, sep_arcsec) of exactly the rows found."""
+    torch = _torch()
+    dev = A.buf.device
+    cap = int(capacity) if capacity is not None else max(1024, int(A.n))
+    for _ in range(2):
+        oa = torch.empty(cap, dtype=torch.int64, device=dev); ob = torch.empty(cap, dtype=torch.int64, device=dev)
+        os_ = torch.empty(cap, dtype=torch.float64, device=dev); cnt = torch.zeros(1, dtype=torch.int64, device=dev)
+        hlc2_crossmatch(A, B, radius_arcsec, mode, oa, ob, os_, cnt)
+        found = int(cnt.item())
+        if found <= cap:
+            return oa[:found], ob[:found], os_[:found]
+        cap = found
+    raise RuntimeError("crossmatch: result count changed between runs")
+
+
+def kernel_launches() -> int:
+    return int(lib().hlc2_kernel_launches())
+
+
+def version() -> str:
+    return lib().hlc2_version().decode()
