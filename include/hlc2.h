@@ -70,7 +70,8 @@ typedef enum {
  *                     search window spans at most 3 zones.
  *   target_occupancy  mean sources per fine cell over the occupied sky; 0 -> 1.0.
  *   cell_arcsec       explicit fine-cell size; 0 -> derived from the catalogue's density
- *                     (max(r_max, sqrt(target_occupancy * occupied area / n))).
+ *                     (max(r_max, sqrt(target_occupancy * occupied area / n))).  Honoured while the cell
+ *                     table stays within max(16 n, 2^25) cells, else coarsened until it fits.
  *   full_sky          non-zero: the grid spans the whole sphere whatever the data extent.
  *   grid_like         if non-NULL, reuse that index's grid exactly (zones, cells, box).  The
  *                     catalogue must lie inside that grid's box (else HLC2_ERR_GRID_MISMATCH).

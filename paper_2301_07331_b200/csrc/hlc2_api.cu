@@ -83,7 +83,11 @@ static void caps(int64_t n, const hlc2_opts& o, size_t* cap_cells, size_t* cap_z
         cell = std::max(cell, o.r_max_arcsec);
         size_t zones = (size_t)ceil(648000.0 / cell) + 2;
         *cap_zones = zones;
-        *cap_cells = (size_t)(kSphereArcsec2 / (cell * cell) * 1.01) + zones + 16;
+        // an explicit cell size is honoured up to a table budget of max(16 n, 2^25) cells; beyond that the
+        // planner coarsens the cells until the table fits
+        double full = kSphereArcsec2 / (cell * cell) * 1.01 + (double)zones + 16.0;
+        double budget = std::max(16.0 * (double)n, 33554432.0);
+        *cap_cells = (size_t)std::min(full, budget);
     } else {
         *cap_cells = (size_t)ceil((double)n / o.target_occupancy * 1.25) + 4096;
         *cap_zones = std::min<size_t>(*cap_cells, (size_t)1 << 20);
