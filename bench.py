@@ -1,0 +1,310 @@
+#!/usr/bin/env python
+"""bench.py -- the measurement contract of the HLC2 cross-match hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C] [--scale S]
+
+A "step" is one pass of the whole hot path over one batch of synthetic input already resident in
+HBM: hlc2_build_index(A) + hlc2_build_index(B) + hlc2_crossmatch(A, B) (all SURVEY 8(a) rows except
+streaming).  Workload at N = 1: configuration 3 of BASELINE.json ("Gaia-like density", A = 100M,
+B = 50M, r = 1 arcsec, all_pairs) -- the configuration north_star's target is quoted on.
+
+One JSON line is printed (rank 0).  `value` = A sources cross-matched per second over the whole step,
+all GPUs together.  north_star allows one GPU only (no sharding, no collectives): with --gpus N > 1
+every rank runs an independent replica on its own GPU ("replicas only", weak scaling).
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the host cores over a bounded sample
+of the same workload; it is a deliberately slow program, reported as a baseline, not a target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "A-sources cross-matched/sec"
+UNIT = "A-sources/s"
+FALLBACK_HBM_GBS = 6650.0       # /opt/skills/guides/B200_PROFILING.md fallback if MEASURED_PEAKS.json is absent
+
+
+def dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("LOCAL_RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+
+
+def peak_hbm():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+def ncu_traffic():
+    """DRAM bytes per launch of the match kernel from the committed ncu --set full capture, or None."""
+    p = os.path.join(ROOT, "profiles", "match_traffic.json")
+    try:
+        return json.load(open(p))
+    except Exception:
+        return None
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []; self.proc = None; self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True); self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def sample_patch(w, ra_lo=0.0, ra_hi=3.6):
+    """Bounded sample of a workload for the CPU legs: both catalogues restricted to an RA slice
+    (same sky density, so per-source work is representative; edge effects ~ r / slice width)."""
+    import hlc2_synth as S
+    ma = (w.A.ra >= ra_lo) & (w.A.ra < ra_hi); mb = (w.B.ra >= ra_lo) & (w.B.ra < ra_hi)
+    return S.Catalogue(w.A.ra[ma], w.A.dec[ma], w.A.id[ma]), S.Catalogue(w.B.ra[mb], w.B.dec[mb], w.B.id[mb])
+
+
+def time_oracle(A, B, radius, mode):
+    import oracle
+    t = time.perf_counter()
+    a, b, s, used = oracle.match(A.ra, A.dec, A.id, B.ra, B.dec, B.id, radius, mode)
+    dt = time.perf_counter() - t
+    return dt, len(a), used
+
+
+def run_reference(args, w, mode):
+    """--impl reference: the oracle, as it stands, on the host cores; each step = the bounded sample."""
+    rank, _, world = dist_env()
+    if rank != 0:
+        return
+    A, B = sample_patch(w, 0.0, args.sample_ra_deg)
+    for _ in range(args.warmup):
+        time_oracle(A, B, w.radius_arcsec, mode)
+    t_tot, used = 0.0, 0
+    for _ in range(args.steps):
+        dt, npairs, used = time_oracle(A, B, w.radius_arcsec, mode)
+        t_tot += dt
+    val = len(A) * args.steps / t_tot
+    sample = f"both catalogues restricted to RA in [0,{args.sample_ra_deg}) deg: {len(A)} x {len(B)} sources, {npairs} rows"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f80 (x87 long double)", "data": "synthetic",
+            "config": {"workload": w.name, "n_a": len(w.A), "n_b": len(w.B), "radius_arcsec": w.radius_arcsec,
+                       "mode": "nearest" if mode else "all_pairs", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--scale", type=float, default=1.0, help="scale the source counts (1.0 = the named configuration)")
+    ap.add_argument("--sample-ra-deg", type=float, default=3.6, help="RA slice of the CPU-baseline sample")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--occupancy", type=float, default=0.0)
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank, local_rank, world = dist_env()
+
+    import hlc2_synth as S
+    if args.impl == "reference" and rank != 0:
+        return 0
+    t0 = time.perf_counter()
+    # replicas: every rank generates its own catalogue (different seed) of the same shape
+    w = S.config(args.config, scale=args.scale, seed=S.BASE_SEED + args.config + 1000 * rank)
+    t_gen = time.perf_counter() - t0
+    mode = 1 if w.modes == ("nearest",) else 0
+    if args.impl == "reference":
+        run_reference(args, w, mode)
+        return 0
+
+    import torch
+    import paper_2301_07331_b200 as P
+    from paper_2301_07331_b200 import build as hb
+    hb.build()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device; there is no CPU fallback"
+    torch.cuda.set_device(local_rank)
+    use_dist = world > 1
+    if use_dist:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    n_a, n_b, r = len(w.A), len(w.B), w.radius_arcsec
+    # pinned host copies (the e2e leg copies from these inside its timed region)
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    hA = [pin(w.A.ra), pin(w.A.dec), pin(w.A.id)]; hB = [pin(w.B.ra), pin(w.B.dec), pin(w.B.id)]
+    dA = [t.cuda(non_blocking=True) for t in hA]; dB = [t.cuda(non_blocking=True) for t in hB]
+    torch.cuda.synchronize()
+
+    opts_a = P.make_opts(r, target_occupancy=args.occupancy); opts_b = P.make_opts(r, target_occupancy=args.occupancy)
+    ib_a, tb_a = P.hlc2_index_sizes(n_a, opts_a); ib_b, tb_b = P.hlc2_index_sizes(n_b, opts_b)
+    buf_a = torch.empty(ib_a, dtype=torch.uint8, device="cuda"); buf_b = torch.empty(ib_b, dtype=torch.uint8, device="cuda")
+    temp = torch.empty(max(tb_a, tb_b), dtype=torch.uint8, device="cuda")
+    cap = int(max(n_a, n_b) * 0.5) + 1024 if mode == 0 else n_a
+    out_a = torch.empty(cap, dtype=torch.int64, device="cuda"); out_b = torch.empty(cap, dtype=torch.int64, device="cuda")
+    out_s = torch.empty(cap, dtype=torch.float64, device="cuda"); cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    h_out = [torch.empty(cap, dtype=torch.int64).pin_memory(), torch.empty(cap, dtype=torch.int64).pin_memory(),
+             torch.empty(cap, dtype=torch.float64).pin_memory()]
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+
+    def step(devA, devB, marks=None):
+        if marks is not None: marks[0].record()
+        ia = P.hlc2_build_index(devA[0], devA[1], devA[2], opts=opts_a, temp=temp, buf=buf_a)
+        if marks is not None: marks[1].record()
+        ib = P.hlc2_build_index(devB[0], devB[1], devB[2], opts=opts_b, temp=temp, buf=buf_b)
+        if marks is not None: marks[2].record()
+        P.hlc2_crossmatch(ia, ib, r, mode, out_a, out_b, out_s, cnt)
+        if marks is not None: marks[3].record()
+        return ia, ib
+
+    def barrier():
+        if use_dist:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        ia, ib = step(dA, dB)
+    torch.cuda.synchronize()
+    found = int(cnt.item())
+    assert found <= cap, f"output capacity {cap} too small for {found} rows"
+    grid_a, grid_b = P.hlc2_grid_describe(ia), P.hlc2_grid_describe(ib)
+
+    # ---- timed region 1: inputs resident in HBM (inputs 3.6 GB >> 126 MB L2, so every step starts cold) ----
+    marks = [[ev() for _ in range(4)] for _ in range(args.steps)]
+    clocks = ClockSampler(local_rank); clocks.start()
+    n0 = P.kernel_launches()
+    barrier()
+    e0, e1 = ev(), ev()
+    e0.record()
+    for k in range(args.steps):
+        step(dA, dB, marks[k])
+    e1.record()
+    barrier()
+    launches = P.kernel_launches() - n0
+    clk = clocks.stop()
+    t_ms = e0.elapsed_time(e1)
+    ph = np.array([[m[0].elapsed_time(m[1]), m[1].elapsed_time(m[2]), m[2].elapsed_time(m[3])] for m in marks])
+    t_build_a, t_build_b, t_match = ph.mean(axis=0)
+
+    # ---- timed region 2 (e2e): host buffers, H2D of the inputs and D2H of the results inside the region ----
+    def e2e_step():
+        da = [t.cuda(non_blocking=True) for t in hA]; db = [t.cuda(non_blocking=True) for t in hB]
+        step(da, db)
+        nf = int(cnt.item())                       # D2H of the count (sync), then of the rows found
+        for src, dst in zip((out_a, out_b, out_s), h_out):
+            dst[:nf].copy_(src[:nf], non_blocking=True)
+        return nf
+    e2e_step(); torch.cuda.synchronize()
+    barrier()
+    g0, g1 = ev(), ev()
+    g0.record()
+    for _ in range(args.steps):
+        nf = e2e_step()
+    g1.record()
+    barrier()
+    t_e2e_ms = g0.elapsed_time(g1)
+    h2d = 24 * (n_a + n_b); d2h = 24 * nf + 8
+
+    if use_dist:
+        tt = torch.tensor([t_ms, t_e2e_ms, t_match], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_ms, t_e2e_ms, t_match_max = tt.tolist()
+        tot = torch.tensor([n_a, found], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+        units, pairs_all = tot.tolist()
+    else:
+        units, pairs_all = float(n_a), float(found)
+
+    if rank == 0:
+        peak, peak_src = peak_hbm()
+        alg_bytes = 32.0 * n_a + 32.0 * n_b + 24.0 * found          # catalogue (sorted SoA) + output bytes
+        achieved = alg_bytes / (t_match * 1e-3) / 1e9
+        tr = ncu_traffic()
+        roof = {"bound": "hbm", "kernel": "k_match (hlc2_crossmatch)", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0, "peak_source": peak_src,
+                "traffic": tr["dram_bytes_per_launch"] if tr else None, "algorithmic_bytes": alg_bytes,
+                "ms_per_launch": float(t_match)}
+        cpu = None
+        if not args.no_cpu_baseline:
+            sa, sb = sample_patch(w, 0.0, args.sample_ra_deg)
+            dt, npairs, used = time_oracle(sa, sb, r, mode)
+            cpu = {"value": len(sa) / dt, "unit": UNIT, "cores": used, "kind": "oracle", "seconds": dt,
+                   "sample": f"both catalogues restricted to RA in [0,{args.sample_ra_deg}) deg: {len(sa)} x {len(sb)} sources, {npairs} rows"}
+        line = {"metric": METRIC, "value": units * args.steps / (t_ms * 1e-3), "unit": UNIT, "n_gpus": world,
+                "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_ms / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+                "config": {"workload": w.name, "n_a": n_a, "n_b": n_b, "radius_arcsec": r,
+                           "mode": "nearest" if mode else "all_pairs", "rows_found": found,
+                           "parallelism": "replicas only (north_star: one GPU, no collectives)" if world > 1 else "1 gpu",
+                           "l2": "inputs (3.6 GB at scale 1) larger than L2; no explicit flush",
+                           "cells_a": grid_a["n_cells"], "cells_b": grid_b["n_cells"], "cell_arcsec_b": grid_b["cell_arcsec"],
+                           "gen_seconds": t_gen},
+                "pairs_per_s": pairs_all * args.steps / (t_ms * 1e-3),
+                "match_phase": {"ms": float(t_match), "a_sources_per_s": n_a / (t_match * 1e-3), "pairs_per_s": found / (t_match * 1e-3)},
+                "phases_ms": {"build_index_A": float(t_build_a), "build_index_B": float(t_build_b), "crossmatch": float(t_match)},
+                "roofline": roof, "cpu_baseline": cpu,
+                "e2e": {"value": units * args.steps / (t_e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+                        "d2h_bytes_per_step": d2h, "ms_per_step": t_e2e_ms / args.steps,
+                        "path": "pinned host -> H2D -> hlc2_build_index x2 -> hlc2_crossmatch -> D2H of count and rows"},
+                "gpu_launches": int(launches), "clocks": clk}
+        print(json.dumps(line), flush=True)
+    if use_dist:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

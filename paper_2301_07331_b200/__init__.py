@@ -133,7 +133,7 @@ def hlc2_index_sizes(n: int, opts: hlc2_opts | None = None):
 
 
 def hlc2_build_index(ra_deg, dec_deg, ids=None, opts: hlc2_opts | None = None, stream=None, temp=None,
-                     like: Index | None = None) -> Index:
+                     like: Index | None = None, buf=None) -> Index:
     """ra_deg, dec_deg: CUDA float64 tensors [n]; ids: CUDA int64 tensor [n] or None (row numbers)."""
     torch = _torch()
     n = int(ra_deg.shape[0])
@@ -146,7 +146,8 @@ def hlc2_build_index(ra_deg, dec_deg, ids=None, opts: hlc2_opts | None = None, s
     if ids is not None:
         assert ids.is_cuda and ids.dtype == torch.int64 and ids.is_contiguous() and ids.shape[0] == n
     ib, tb = hlc2_index_sizes(n, opts)
-    buf = torch.empty(ib, dtype=torch.uint8, device=ra_deg.device)
+    if buf is None or buf.numel() < ib:
+        buf = torch.empty(ib, dtype=torch.uint8, device=ra_deg.device)
     if temp is None or temp.numel() < tb:
         temp = torch.empty(tb, dtype=torch.uint8, device=ra_deg.device)
     out = ctypes.c_void_p()
