@@ -60,7 +60,7 @@ typedef enum {
     HLC2_ERR_BAD_COORD = -4,         /* a non-finite coordinate or |dec| > 90 was found (hlc2_index_status) */
     HLC2_ERR_CUDA = -5,              /* a CUDA runtime call failed; see hlc2_last_cuda_error */
     HLC2_ERR_GRID_MISMATCH = -6,     /* opts.grid_like: the catalogue does not fit inside that grid's box */
-    HLC2_ERR_TOO_MANY = -7           /* n >= 2^32 - 1 sources in one index (stream the catalogue instead) */
+    HLC2_ERR_TOO_MANY = -7           /* n >= 2^30 sources in one index (stream the catalogue instead) */
 } hlc2_status;
 
 /*

@@ -38,10 +38,10 @@ struct HostGrid {
 };
 
 struct Layout {           // byte offsets inside the index buffer
-    size_t x, y, z, id, key, cell_start, n_ra, cell_base, stats, total;
-    size_t cap_cells, cap_zones, n_pad;
+    size_t x, y, z, id, key, cell_start, n_ra, cell_base, tiles, n_tiles, stats, total;
+    size_t cap_cells, cap_zones, cap_tiles, n_pad;
 };
-struct TempLayout { size_t key_b, perm_a, perm_b, counts, partials, total; };
+struct TempLayout { size_t key_b, perm_a, perm_b, rec, digit_hist, digit_base, ticket, status, big, tile_first, total; };
 
 struct hlc2_index {
     uint32_t magic;
@@ -103,9 +103,12 @@ static Layout make_layout(int64_t n, const hlc2_opts& o) {
     L.z = off; off += align_up(L.n_pad * 8);
     L.id = off; off += align_up(L.n_pad * 8);
     L.key = off; off += align_up(L.n_pad * 4);
-    L.cell_start = off; off += align_up((L.cap_cells + 1) * 4);
+    L.cell_start = off; off += align_up((L.cap_cells + 1) * 4 + 64);   // slack: bulk copies round up to 16 bytes
     L.n_ra = off; off += align_up(L.cap_zones * 4);
     L.cell_base = off; off += align_up((L.cap_zones + 1) * 4);
+    L.cap_tiles = (size_t)n / kTile + L.cap_zones + 1;
+    L.tiles = off; off += align_up(L.cap_tiles * sizeof(TileDesc));
+    L.n_tiles = off; off += 256;
     L.stats = off; off += align_up(sizeof(Stats));
     L.total = off;
     return L;
@@ -115,10 +118,13 @@ static TempLayout make_temp(int64_t n, const Layout& L) {
     T.key_b = off; off += align_up(L.n_pad * 4);
     T.perm_a = off; off += align_up(L.n_pad * 4);
     T.perm_b = off; off += align_up(L.n_pad * 4);
-    size_t ce = sort_counts_entries((uint32_t)n);
-    T.counts = off; off += align_up((ce + 256) * 4);
-    size_t pe = scan_partials_entries(std::max(ce, L.cap_cells + 1));
-    T.partials = off; off += align_up((pe + 1024) * 4);
+    T.rec = off; off += align_up(L.n_pad * sizeof(Rec));
+    T.digit_hist = off; off += align_up((size_t)kMaxPasses * kRadix * 4);
+    T.digit_base = off; off += align_up((size_t)kMaxPasses * kRadix * 4);
+    T.ticket = off; off += 256;
+    T.status = off; off += align_up((size_t)kMaxPasses * sort_tiles((uint32_t)n) * kRadix * 4 + 256);
+    T.big = off; off += align_up((3 * cell_big_cap(L.cap_cells) + 1) * 4);
+    T.tile_first = off; off += align_up((L.cap_zones + 2) * 4);
     T.total = off;
     return T;
 }
@@ -190,7 +196,7 @@ static GridView grid_view(const hlc2_index* ix) {
     GridView v;
     v.n_ra = (const int32_t*)(ix->d_buf + ix->lay.n_ra);
     v.cell_base = (const uint32_t*)(ix->d_buf + ix->lay.cell_base);
-    v.dec_lo = ix->grid.dec_lo; v.inv_h = 1.0 / ix->grid.h; v.ra0 = ix->grid.ra0; v.span = ix->grid.span;
+    v.dec_lo = ix->grid.dec_lo; v.h = ix->grid.h; v.inv_h = 1.0 / ix->grid.h; v.ra0 = ix->grid.ra0; v.span = ix->grid.span;
     v.inv_span = 1.0 / ix->grid.span; v.dec_min = ix->grid.dec_min; v.dec_max = ix->grid.dec_max;
     v.n_zones = (int32_t)ix->grid.n_zones; v.n_cells = ix->grid.n_cells();
     return v;
@@ -200,7 +206,9 @@ static IndexView index_view(const hlc2_index* ix) {
     v.x = (const double*)(ix->d_buf + ix->lay.x); v.y = (const double*)(ix->d_buf + ix->lay.y);
     v.z = (const double*)(ix->d_buf + ix->lay.z); v.id = (const int64_t*)(ix->d_buf + ix->lay.id);
     v.cell_start = (const uint32_t*)(ix->d_buf + ix->lay.cell_start);
+    v.tiles = (const TileDesc*)(ix->d_buf + ix->lay.tiles); v.n_tiles = (const uint32_t*)(ix->d_buf + ix->lay.n_tiles);
     v.g = grid_view(ix); v.n = (uint32_t)ix->n;
+    v.tile_cap = (uint32_t)((size_t)ix->n / kTile + (size_t)ix->grid.n_zones + 1);
     return v;
 }
 
@@ -277,22 +285,27 @@ int hlc2_build_index(const double* d_ra, const double* d_dec, const int64_t* d_i
     }
     GridView gv = grid_view(ix);
 
-    // (a1) keys -> (a2) radix sort (key, row) -> (a3) gather -> (a4) cell table
+    // (a1) keys + packed records + digit counts -> (a2) radix sort (key, row) -> (a3) gather -> (a4) cell table, tiles
     uint32_t n_cells = g.n_cells();
     int key_bits = 1; while (key_bits < 32 && (1ull << key_bits) < (unsigned long long)n_cells) ++key_bits;
-    int passes = (key_bits + 7) / 8;
+    int passes = radix_passes(key_bits);
     uint32_t* key_idx = (uint32_t*)(buf + L.key);           // the sorted keys must end up here
     uint32_t* key_tmp = (uint32_t*)(tmp + T.key_b);
     uint32_t* ka = (passes & 1) ? key_tmp : key_idx;        // start buffer chosen by pass parity
     uint32_t* kb = (passes & 1) ? key_idx : key_tmp;
     uint32_t* pa = (uint32_t*)(tmp + T.perm_a); uint32_t* pb = (uint32_t*)(tmp + T.perm_b);
-    launch_keys(d_ra, d_dec, nn, gv, ka, s);
-    int where = launch_radix_sort(ka, kb, pa, pb, nn, key_bits, (uint32_t*)(tmp + T.counts), 0,
-                                  (uint32_t*)(tmp + T.partials), s);
+    Rec* rec = (Rec*)(tmp + T.rec);
+    uint32_t* digit_hist = (uint32_t*)(tmp + T.digit_hist);
+    if (cudaMemsetAsync(digit_hist, 0, (size_t)kMaxPasses * kRadix * 4, s) != cudaSuccess) { t_last_cuda = cudaGetLastError(); return fail(HLC2_ERR_CUDA); }
+    launch_keys_pack(d_ra, d_dec, d_id, nn, gv, passes, ka, rec, digit_hist, s);
+    int where = launch_radix_sort(ka, kb, pa, pb, nn, key_bits, digit_hist, (uint32_t*)(tmp + T.digit_base),
+                                  (uint32_t*)(tmp + T.status), (uint32_t*)(tmp + T.ticket), s);
     const uint32_t* perm = where ? pb : pa;
-    launch_gather(d_ra, d_dec, d_id, perm, nn, (double*)(buf + L.x), (double*)(buf + L.y), (double*)(buf + L.z),
-                  (int64_t*)(buf + L.id), s);
-    launch_cell_table(key_idx, nn, n_cells, (uint32_t*)(buf + L.cell_start), (uint32_t*)(tmp + T.partials), s);
+    launch_gather(rec, perm, nn, (double*)(buf + L.x), (double*)(buf + L.y), (double*)(buf + L.z), (int64_t*)(buf + L.id), s);
+    launch_cell_table(key_idx, nn, n_cells, (uint32_t*)(buf + L.cell_start), (uint32_t*)(tmp + T.big), s);
+    launch_tiles((const uint32_t*)(buf + L.cell_start), gv.cell_base, (uint32_t)g.n_zones, key_idx,
+                 (uint32_t)((size_t)n / kTile + (size_t)g.n_zones + 1), (uint32_t*)(tmp + T.tile_first),
+                 (TileDesc*)(buf + L.tiles), (uint32_t*)(buf + L.n_tiles), s);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) { t_last_cuda = e; return fail(HLC2_ERR_CUDA); }
     // the host grid vectors were copied with cudaMemcpyAsync from pageable memory: that call
@@ -342,23 +355,25 @@ int hlc2_index_arrays(const hlc2_index* idx, const double** d_x, const double** 
 
 int hlc2_crossmatch_sizes(const hlc2_index* A, const hlc2_index* B, size_t* temp_bytes) {
     if (!A || !B || A->magic != kMagic || B->magic != kMagic || !temp_bytes) return HLC2_ERR_INVALID_ARG;
-    *temp_bytes = 0;
+    *temp_bytes = match_temp_bytes(index_view(A), index_view(B));
     return HLC2_OK;
 }
 
 int hlc2_crossmatch(const hlc2_index* A, const hlc2_index* B, double radius_arcsec, int mode,
                     int64_t* d_out_idA, int64_t* d_out_idB, double* d_out_sep, int64_t capacity,
                     unsigned long long* d_count, void* d_temp, size_t temp_bytes, void* cuda_stream) {
-    (void)d_temp; (void)temp_bytes;
     if (!A || !B || A->magic != kMagic || B->magic != kMagic || !d_count || capacity < 0 ||
         (capacity > 0 && (!d_out_idA || !d_out_idB || !d_out_sep)) ||
         (mode != HLC2_ALL_PAIRS && mode != HLC2_NEAREST) ||
         !(radius_arcsec > 0.0) || !std::isfinite(radius_arcsec)) return HLC2_ERR_INVALID_ARG;
     if (radius_arcsec > std::min(A->opts.r_max_arcsec, B->opts.r_max_arcsec)) return HLC2_ERR_RADIUS_TOO_LARGE;
+    IndexView va = index_view(A), vb = index_view(B);
+    size_t need = match_temp_bytes(va, vb);
+    if (need > 0 && (!d_temp || temp_bytes < need)) return HLC2_ERR_BUFFER_TOO_SMALL;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     CU(cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), s));
-    launch_match(index_view(A), index_view(B), radius_arcsec, mode, d_out_idA, d_out_idB, d_out_sep,
-                 (unsigned long long)capacity, d_count, s);
+    launch_match(va, vb, radius_arcsec, mode, d_out_idA, d_out_idB, d_out_sep,
+                 (unsigned long long)capacity, d_count, d_temp, s);
     CU(cudaGetLastError());
     return HLC2_OK;
 }
@@ -376,7 +391,7 @@ const char* hlc2_strerror(int status) {
         case HLC2_ERR_BAD_COORD: return "non-finite coordinate or |dec| > 90 in the catalogue";
         case HLC2_ERR_CUDA: return "CUDA runtime error (see hlc2_last_cuda_error)";
         case HLC2_ERR_GRID_MISMATCH: return "catalogue does not fit inside the grid_like index's RA box";
-        case HLC2_ERR_TOO_MANY: return "too many sources for one index (>= 2^32 - 1)";
+        case HLC2_ERR_TOO_MANY: return "too many sources for one index (>= 2^30)";
         default: return "unknown status";
     }
 }

@@ -1,6 +1,18 @@
-// hlc2_build.cu -- index-build kernels (NS (a)): extent statistics, cell keys,
-// LSD radix sort of (key, row), gather into SoA unit vectors, cell offset table by scan.
-// All kernels are HBM-bound streaming passes; grids are sized in multiples of the SM count.
+// hlc2_build.cu -- index-build kernels (NS (a)).
+//
+//   k_stats        (a1) validity, dec extent, coarse RA occupancy            16 B/source read
+//   k_keys_pack    (a1) cell key + unit vector; packs a 32-byte AoS record {x,y,z,id} in input order and
+//                       accumulates the digit histograms of every radix pass  24 B read, 36 B written
+//   k_digit_scan   (a2) exclusive scan of the per-pass digit histograms (one CTA)
+//   k_onesweep     (a2) one LSD radix pass over (key, row): chained-scan ("decoupled look-back") of tile digit
+//                       counts, ranks by warp match, smem reorder so that every digit run is written
+//                       coalesced                                              8 B read, 8 B written per pass
+//   k_gather       (a3) one 32-byte sector per source (the packed record) -> cell-sorted SoA x,y,z,id
+//   k_cell_fill    (a4) run boundaries of the sorted keys -> cell_start[] (also for empty cells), long empty
+//                       runs handed to k_cell_fill_big
+//   k_zone_tiles, k_tile_desc (a4) tile descriptors: runs of <= kTile consecutive sources inside one zone
+//
+// All of them are HBM-bound streaming passes; grids are multiples of the SM count.
 #include <string.h>
 #include <algorithm>
 
@@ -9,7 +21,7 @@
 namespace hlc2 {
 
 static int g_sm_count = 0;
-static int sm_count() {
+int sm_count() {
     if (!g_sm_count) {
         int dev = 0; cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -70,244 +82,10 @@ void launch_stats(const double* ra, const double* dec, uint32_t n, Stats* d_stat
 }
 
 // ------------------------------------------------------------------------------------------
-// (a1) cell keys
-// ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256)
-k_keys(const double* __restrict__ ra, const double* __restrict__ dec, uint32_t n, GridView g, uint32_t* __restrict__ keys) {
-    for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (size_t)gridDim.x * 256) {
-        double a = __ldg(ra + i), d = __ldg(dec + i);
-        uint32_t key = 0;
-        if (coord_ok(a, d)) {
-            int z = zone_of(g, d);
-            int nra = __ldg(g.n_ra + z);
-            key = __ldg(g.cell_base + z) + (uint32_t)cell_of_u(g, box_u(g, norm_ra(a)), nra);
-        }
-        keys[i] = key;
-    }
-}
-
-void launch_keys(const double* ra, const double* dec, uint32_t n, GridView g, uint32_t* keys, cudaStream_t s) {
-    if (n == 0) return;
-    int blocks = (int)std::min<size_t>(((size_t)n + 255) / 256, (size_t)sm_count() * 16);
-    k_keys<<<blocks, 256, 0, s>>>(ra, dec, n, g, keys); count_launch();
-}
-
-// ------------------------------------------------------------------------------------------
-// device-wide scan (three kernels: block reduce, scan of partials, block scan with carry-in)
-//   Sum, forward, exclusive  -> radix-sort digit offsets
-//   Min, reverse, inclusive  -> cell table (next occupied cell's first row)
-// ------------------------------------------------------------------------------------------
-constexpr int kScanThreads = 256;
-constexpr int kScanItems = 16;
-constexpr int kScanChunk = kScanThreads * kScanItems;
-
-struct OpSum { static __device__ __forceinline__ uint32_t id() { return 0u; }
-               static __device__ __forceinline__ uint32_t ap(uint32_t a, uint32_t b) { return a + b; } };
-struct OpMin { static __device__ __forceinline__ uint32_t id() { return 0xFFFFFFFFu; }
-               static __device__ __forceinline__ uint32_t ap(uint32_t a, uint32_t b) { return min(a, b); } };
-
-size_t scan_partials_entries(size_t m) { return (m + kScanChunk - 1) / kScanChunk + 1; }
-
-// inclusive scan of one value per thread across the block; returns the inclusive prefix, *total = block aggregate
-template <class Op>
-__device__ __forceinline__ uint32_t block_scan_incl(uint32_t v, uint32_t* total, uint32_t* sm /*[33]*/) {
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xffffffffu, v, o); if (lane >= o) v = Op::ap(t, v); }
-    if (lane == 31) sm[w] = v;
-    __syncthreads();
-    if (w == 0) {
-        uint32_t t = lane < (int)(blockDim.x >> 5) ? sm[lane] : Op::id();
-        for (int o = 1; o < 32; o <<= 1) { uint32_t u = __shfl_up_sync(0xffffffffu, t, o); if (lane >= o) t = Op::ap(u, t); }
-        sm[lane] = t;
-        if (lane == 31) sm[32] = t;
-    }
-    __syncthreads();
-    if (w > 0) v = Op::ap(sm[w - 1], v);
-    *total = sm[32];
-    __syncthreads();
-    return v;
-}
-
-template <class Op, bool Rev>
-__global__ void __launch_bounds__(kScanThreads)
-k_scan_reduce(const uint32_t* __restrict__ a, size_t m, uint32_t* __restrict__ partials) {
-    __shared__ uint32_t sm[33];
-    size_t base = (size_t)blockIdx.x * kScanChunk;
-    uint32_t acc = Op::id();
-#pragma unroll
-    for (int r = 0; r < kScanItems; ++r) {
-        size_t i = base + (size_t)r * kScanThreads + threadIdx.x;
-        if (i < m) acc = Op::ap(acc, a[Rev ? m - 1 - i : i]);
-    }
-    uint32_t tot; block_scan_incl<Op>(acc, &tot, sm);
-    if (threadIdx.x == 0) partials[blockIdx.x] = tot;
-}
-
-// single block: partials[b] <- exclusive scan over blocks
-template <class Op>
-__global__ void __launch_bounds__(1024)
-k_scan_partials(uint32_t* __restrict__ partials, size_t nb) {
-    __shared__ uint32_t sm[33];
-    uint32_t carry = Op::id();
-    for (size_t base = 0; base < nb; base += 1024) {
-        size_t i = base + threadIdx.x;
-        uint32_t v = i < nb ? partials[i] : Op::id();
-        uint32_t tot; uint32_t inc = block_scan_incl<Op>(v, &tot, sm);
-        // exclusive = carry (op) inclusive-of-previous
-        uint32_t prev = __shfl_up_sync(0xffffffffu, inc, 1);
-        __shared__ uint32_t last[32];
-        if ((threadIdx.x & 31) == 31) last[threadIdx.x >> 5] = inc;
-        __syncthreads();
-        uint32_t ex = (threadIdx.x & 31) ? prev : (threadIdx.x ? last[(threadIdx.x >> 5) - 1] : Op::id());
-        if (i < nb) partials[i] = Op::ap(carry, ex);
-        carry = Op::ap(carry, tot);
-        __syncthreads();
-    }
-}
-
-template <class Op, bool Rev, bool Incl>
-__global__ void __launch_bounds__(kScanThreads)
-k_scan_apply(uint32_t* __restrict__ a, size_t m, const uint32_t* __restrict__ partials) {
-    __shared__ uint32_t sm[33];
-    // thread t owns kScanItems consecutive logical entries
-    size_t base = (size_t)blockIdx.x * kScanChunk + (size_t)threadIdx.x * kScanItems;
-    uint32_t v[kScanItems];
-    uint32_t acc = Op::id();
-#pragma unroll
-    for (int r = 0; r < kScanItems; ++r) {
-        size_t i = base + r;
-        v[r] = i < m ? a[Rev ? m - 1 - i : i] : Op::id();
-        acc = Op::ap(acc, v[r]);
-    }
-    uint32_t tot; uint32_t inc = block_scan_incl<Op>(acc, &tot, sm);
-    // exclusive prefix of this thread = inclusive prefix of the previous thread
-    __shared__ uint32_t s_inc[kScanThreads];
-    s_inc[threadIdx.x] = inc;
-    __syncthreads();
-    uint32_t run = Op::ap(partials[blockIdx.x], threadIdx.x ? s_inc[threadIdx.x - 1] : Op::id());
-#pragma unroll
-    for (int r = 0; r < kScanItems; ++r) {
-        size_t i = base + r;
-        uint32_t nxt = Op::ap(run, v[r]);
-        if (i < m) a[Rev ? m - 1 - i : i] = Incl ? nxt : run;
-        run = nxt;
-    }
-}
-
-template <class Op, bool Rev, bool Incl>
-static void device_scan(uint32_t* a, size_t m, uint32_t* partials, cudaStream_t s) {
-    if (m == 0) return;
-    size_t nb = (m + kScanChunk - 1) / kScanChunk;
-    k_scan_reduce<Op, Rev><<<(unsigned)nb, kScanThreads, 0, s>>>(a, m, partials);
-    k_scan_partials<Op><<<1, 1024, 0, s>>>(partials, nb);
-    k_scan_apply<Op, Rev, Incl><<<(unsigned)nb, kScanThreads, 0, s>>>(a, m, partials);
-    count_launch(3);
-}
-
-// ------------------------------------------------------------------------------------------
-// (a2) LSD radix sort of (key, row), 8-bit digits: per-tile digit histogram -> device scan ->
-// stable scatter.  Tile = 256 threads x 16 keys; warp w of a tile owns 512 consecutive keys.
-// ------------------------------------------------------------------------------------------
-constexpr int kSortThreads = 256;
-constexpr int kSortItems = 16;
-constexpr int kSortTile = kSortThreads * kSortItems;   // 4096
-constexpr int kSortWarps = kSortThreads / 32;
-
-size_t sort_counts_entries(uint32_t n) { return 256 * (((size_t)n + kSortTile - 1) / kSortTile); }
-
-__global__ void __launch_bounds__(kSortThreads)
-k_sort_hist(const uint32_t* __restrict__ keys, uint32_t n, int shift, uint32_t mask,
-            uint32_t* __restrict__ counts, uint32_t n_tiles) {
-    __shared__ uint32_t hist[256];
-    hist[threadIdx.x] = 0;
-    __syncthreads();
-    size_t base = (size_t)blockIdx.x * kSortTile;
-#pragma unroll
-    for (int r = 0; r < kSortItems; ++r) {
-        size_t i = base + (size_t)r * kSortThreads + threadIdx.x;
-        bool ok = i < n;
-        uint32_t d = ok ? ((__ldg(keys + i) >> shift) & mask) : 0xFFFFFFFFu;
-        unsigned peers = __match_any_sync(0xffffffffu, d);
-        if (ok && (peers & ((1u << (threadIdx.x & 31)) - 1)) == 0) atomicAdd(&hist[d], (uint32_t)__popc(peers));
-    }
-    __syncthreads();
-    counts[(size_t)threadIdx.x * n_tiles + blockIdx.x] = hist[threadIdx.x];
-}
-
-template <bool FirstPass>
-__global__ void __launch_bounds__(kSortThreads)
-k_sort_scatter(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals, uint32_t n, int shift, uint32_t mask,
-               const uint32_t* __restrict__ offs, uint32_t n_tiles,
-               uint32_t* __restrict__ out_keys, uint32_t* __restrict__ out_vals) {
-    __shared__ uint32_t wh[kSortWarps][256];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    for (int i = threadIdx.x; i < kSortWarps * 256; i += kSortThreads) (&wh[0][0])[i] = 0;
-    __syncthreads();
-    const size_t base = (size_t)blockIdx.x * kSortTile + (size_t)w * (kSortItems * 32) + lane;
-    uint32_t k[kSortItems], v[kSortItems], rk[kSortItems];
-#pragma unroll
-    for (int r = 0; r < kSortItems; ++r) {
-        size_t i = base + (size_t)r * 32;
-        k[r] = i < n ? __ldg(keys + i) : 0xFFFFFFFFu;
-        v[r] = FirstPass ? (uint32_t)i : (i < n ? __ldg(vals + i) : 0u);
-    }
-    const unsigned lt = (1u << lane) - 1;
-#pragma unroll
-    for (int r = 0; r < kSortItems; ++r) {
-        bool ok = base + (size_t)r * 32 < n;
-        uint32_t d = ok ? ((k[r] >> shift) & mask) : 0xFFFFFFFFu;
-        unsigned peers = __match_any_sync(0xffffffffu, d);
-        uint32_t old = ok ? wh[w][d] : 0u;
-        __syncwarp();
-        if (ok && (peers & lt) == 0) wh[w][d] = old + (uint32_t)__popc(peers);
-        __syncwarp();
-        rk[r] = old + (uint32_t)__popc(peers & lt);
-    }
-    __syncthreads();
-    {   // digit d = threadIdx.x: exclusive scan over the warps of this tile, plus the tile's global offset
-        uint32_t run = __ldg(offs + (size_t)threadIdx.x * n_tiles + blockIdx.x);
-#pragma unroll
-        for (int ww = 0; ww < kSortWarps; ++ww) { uint32_t t = wh[ww][threadIdx.x]; wh[ww][threadIdx.x] = run; run += t; }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int r = 0; r < kSortItems; ++r) {
-        if (base + (size_t)r * 32 < n) {
-            uint32_t d = (k[r] >> shift) & mask;
-            uint32_t dst = wh[w][d] + rk[r];
-            out_keys[dst] = k[r];
-            out_vals[dst] = v[r];
-        }
-    }
-}
-
-int launch_radix_sort(uint32_t* keys_a, uint32_t* keys_b, uint32_t* val_a, uint32_t* val_b, uint32_t n,
-                      int key_bits, uint32_t* d_counts, size_t counts_entries, uint32_t* d_partials, cudaStream_t s) {
-    if (n == 0) return 0;
-    if (key_bits < 1) key_bits = 1;
-    int passes = (key_bits + 7) / 8;
-    uint32_t n_tiles = (uint32_t)(((size_t)n + kSortTile - 1) / kSortTile);
-    (void)counts_entries;
-    uint32_t *ki = keys_a, *ko = keys_b, *vi = val_a, *vo = val_b;
-    for (int p = 0; p < passes; ++p) {
-        int shift = 8 * p;
-        int bits = std::min(8, key_bits - shift);
-        uint32_t mask = (1u << bits) - 1u;
-        k_sort_hist<<<n_tiles, kSortThreads, 0, s>>>(ki, n, shift, mask, d_counts, n_tiles); count_launch();
-        device_scan<OpSum, false, false>(d_counts, (size_t)256 * n_tiles, d_partials, s);
-        if (p == 0) k_sort_scatter<true><<<n_tiles, kSortThreads, 0, s>>>(ki, vi, n, shift, mask, d_counts, n_tiles, ko, vo);
-        else        k_sort_scatter<false><<<n_tiles, kSortThreads, 0, s>>>(ki, vi, n, shift, mask, d_counts, n_tiles, ko, vo);
-        count_launch();
-        uint32_t* t = ki; ki = ko; ko = t; t = vi; vi = vo; vo = t;
-    }
-    return passes & 1;
-}
-
-// ------------------------------------------------------------------------------------------
-// (a3) gather into cell order + fp64 unit vectors.
-// Accuracy: RA is reduced to |t| <= 45 deg in the degree domain (t = ra - 90 rint(ra/90) is exact),
-// Dec uses the colatitude 90 - |dec| (exact) beyond 45 deg, so the radian conversion never rounds
-// an angle larger than pi/4; unit-vector chords are then good to ~5e-11 arcsec.
+// (a1) cell key + unit vector + packed record + digit histograms
+// Accuracy of the unit vector: RA is reduced to |t| <= 45 deg in the degree domain (t = ra - 90 rint(ra/90) is
+// exact), Dec uses the colatitude 90 - |dec| (exact) beyond 45 deg, so the radian conversion never rounds an
+// angle larger than pi/4; unit-vector chords are then good to ~5e-11 arcsec.
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ void unit_vector(double ra_norm, double dec, double& x, double& y, double& z) {
     const double D2R = 0.017453292519943295;   // pi / 180
@@ -324,46 +102,339 @@ __device__ __forceinline__ void unit_vector(double ra_norm, double dec, double& 
     x = cd * ca; y = cd * sa; z = sd;
 }
 
+constexpr int kKeyThreads = 256;
+
+__global__ void __launch_bounds__(kKeyThreads)
+k_keys_pack(const double* __restrict__ ra, const double* __restrict__ dec, const int64_t* __restrict__ id, uint32_t n,
+            GridView g, int passes, uint32_t* __restrict__ keys, Rec* __restrict__ rec, uint32_t* __restrict__ digit_hist) {
+    __shared__ uint32_t hist[kMaxPasses * kRadix];
+    for (int i = threadIdx.x; i < kMaxPasses * kRadix; i += kKeyThreads) hist[i] = 0;
+    __syncthreads();
+    for (size_t i = (size_t)blockIdx.x * kKeyThreads + threadIdx.x; i < n; i += (size_t)gridDim.x * kKeyThreads) {
+        double a = __ldg(ra + i), d = __ldg(dec + i);
+        long long v = id ? (long long)__ldg(id + i) : (long long)i;
+        uint32_t key = 0;
+        double ux = 0.0, uy = 0.0, uz = 2.0;       // bad coordinate: a point no chord test can reach
+        if (coord_ok(a, d)) {
+            double an = norm_ra(a);
+            int z = zone_of(g, d);
+            int nra = __ldg(g.n_ra + z);
+            key = __ldg(g.cell_base + z) + (uint32_t)cell_of_u(g, box_u(g, an), nra);
+            unit_vector(an, d, ux, uy, uz);
+        }
+        keys[i] = key;
+        double2* o = reinterpret_cast<double2*>(rec + i);
+        o[0] = make_double2(ux, uy);
+        o[1] = make_double2(uz, __longlong_as_double(v));
+        for (int p = 0; p < passes; ++p) atomicAdd(&hist[p * kRadix + ((key >> (p * kRadixBits)) & (kRadix - 1))], 1u);
+    }
+    __syncthreads();
+    for (int i = threadIdx.x; i < passes * kRadix; i += kKeyThreads)
+        if (hist[i]) atomicAdd(&digit_hist[i], hist[i]);
+}
+
+void launch_keys_pack(const double* ra, const double* dec, const int64_t* id, uint32_t n, GridView g, int passes,
+                      uint32_t* keys, Rec* rec, uint32_t* digit_hist, cudaStream_t s) {
+    if (n == 0) return;
+    int blocks = (int)std::min<size_t>(((size_t)n + kKeyThreads - 1) / kKeyThreads, (size_t)sm_count() * 8);
+    k_keys_pack<<<blocks, kKeyThreads, 0, s>>>(ra, dec, id, n, g, passes, keys, rec, digit_hist); count_launch();
+}
+
+// ------------------------------------------------------------------------------------------
+// block-wide inclusive scan of one value per thread (any multiple of 32 threads up to 1024)
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t block_scan_incl(uint32_t v, uint32_t* total, uint32_t* sm /*[33]*/) {
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int o = 1; o < 32; o <<= 1) { uint32_t t = __shfl_up_sync(0xffffffffu, v, o); if (lane >= o) v += t; }
+    if (lane == 31) sm[w] = v;
+    __syncthreads();
+    if (w == 0) {
+        uint32_t t = lane < (int)(blockDim.x >> 5) ? sm[lane] : 0u;
+        for (int o = 1; o < 32; o <<= 1) { uint32_t u = __shfl_up_sync(0xffffffffu, t, o); if (lane >= o) t += u; }
+        sm[lane] = t;
+        if (lane == 31) sm[32] = t;
+    }
+    __syncthreads();
+    if (w > 0) v += sm[w - 1];
+    *total = sm[32];
+    __syncthreads();
+    return v;
+}
+
+// ------------------------------------------------------------------------------------------
+// (a2) LSD radix sort of (key, row): 9-bit digits, one kernel per pass.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kRadix)
+k_digit_scan(const uint32_t* __restrict__ digit_hist, uint32_t* __restrict__ digit_base, int passes) {
+    __shared__ uint32_t sm[33];
+    for (int p = 0; p < passes; ++p) {
+        uint32_t c = digit_hist[p * kRadix + threadIdx.x], tot;
+        uint32_t inc = block_scan_incl(c, &tot, sm);
+        digit_base[p * kRadix + threadIdx.x] = inc - c;
+    }
+}
+
+constexpr int kOsThreads = 512;                 // == kRadix: thread d owns digit d in the tile-level scans
+constexpr int kOsItems = 12;                    // even
+constexpr int kOsTile = kOsThreads * kOsItems;  // 6144 keys per tile
+constexpr int kOsWarps = kOsThreads / 32;
+constexpr uint32_t kFlagAgg = 1u << 30, kFlagIncl = 2u << 30, kFlagMask = 3u << 30;
+constexpr size_t kOsSmem = (size_t)(kOsWarps * kRadix + 2 * kOsTile) * 4;
+static_assert(kOsThreads == kRadix, "one thread per digit");
+
+size_t sort_tiles(uint32_t n) { return ((size_t)n + kOsTile - 1) / kOsTile; }
+
+template <bool FirstPass>
+__global__ void __launch_bounds__(kOsThreads, 2)
+k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals, uint32_t n, int shift, uint32_t mask,
+           const uint32_t* __restrict__ digit_base, volatile uint32_t* __restrict__ status, uint32_t* __restrict__ ticket,
+           uint32_t* __restrict__ out_keys, uint32_t* __restrict__ out_vals) {
+    extern __shared__ uint32_t dsm[];
+    uint32_t* wh = dsm;                            // [kOsWarps][kRadix] per-warp digit counters -> offsets
+    uint32_t* s_keys = dsm + kOsWarps * kRadix;    // [kOsTile]
+    uint32_t* s_vals = s_keys + kOsTile;           // [kOsTile]
+    __shared__ uint32_t s_tile, s_scan[33];
+    __shared__ uint32_t s_gbase[kRadix];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+
+    // tiles are taken in ticket order, so every predecessor of a running tile has itself started: the
+    // look-back below can only wait on CTAs that are resident or finished
+    if (threadIdx.x == 0) s_tile = atomicAdd(ticket, 1u);
+    for (int i = threadIdx.x; i < kOsWarps * kRadix; i += kOsThreads) wh[i] = 0;
+    __syncthreads();
+    const uint32_t tile = s_tile;
+    const size_t tile_base = (size_t)tile * kOsTile;
+    const uint32_t cnt = (uint32_t)min((size_t)kOsTile, (size_t)n - tile_base);
+
+    // warp w owns kOsItems*32 consecutive keys; item r of lane l is key (w*kOsItems + r)*32 + l of the tile
+    const size_t base = tile_base + (size_t)w * (kOsItems * 32) + lane;
+    uint32_t k[kOsItems], v[kOsItems], rk[kOsItems / 2];      // ranks (< kOsTile) packed two per register
+#pragma unroll
+    for (int r = 0; r < kOsItems; ++r) {
+        size_t i = base + (size_t)r * 32;
+        k[r] = i < n ? __ldg(keys + i) : 0xFFFFFFFFu;
+        v[r] = FirstPass ? (uint32_t)i : (i < n ? __ldg(vals + i) : 0u);
+    }
+    const unsigned lt = (1u << lane) - 1;
+    uint32_t* mywh = wh + w * kRadix;
+#pragma unroll
+    for (int r = 0; r < kOsItems; ++r) {
+        const bool ok = base + (size_t)r * 32 < n;
+        const uint32_t d = ok ? ((k[r] >> shift) & mask) : 0xFFFFFFFFu;
+        const unsigned peers = __match_any_sync(0xffffffffu, d);
+        const uint32_t old = ok ? mywh[d] : 0u;
+        __syncwarp();
+        if (ok && (peers & lt) == 0) mywh[d] = old + (uint32_t)__popc(peers);
+        __syncwarp();
+        const uint32_t rank = old + (uint32_t)__popc(peers & lt);
+        if (r & 1) rk[r >> 1] |= rank << 16; else rk[r >> 1] = rank;
+    }
+    __syncthreads();
+
+    // digit d = threadIdx.x: exclusive scan over the warps, tile count, chained scan over the tiles
+    const int dgt = threadIdx.x;
+    uint32_t c = 0;
+#pragma unroll
+    for (int ww = 0; ww < kOsWarps; ++ww) { uint32_t t = wh[ww * kRadix + dgt]; wh[ww * kRadix + dgt] = c; c += t; }
+    volatile uint32_t* my_status = status + (size_t)tile * kRadix + dgt;
+    *my_status = c | (tile == 0 ? kFlagIncl : kFlagAgg);
+    uint32_t tot;
+    const uint32_t loc = block_scan_incl(c, &tot, s_scan) - c;      // first position of digit d in the sorted tile
+    uint32_t excl = 0;
+    if (tile > 0) {
+        volatile uint32_t* p = my_status - kRadix;
+        for (;;) {
+            uint32_t sv = *p;
+            if ((sv & kFlagMask) == 0) continue;
+            excl += sv & ~kFlagMask;
+            if (sv & kFlagIncl) break;
+            p -= kRadix;
+        }
+        *my_status = (excl + c) | kFlagIncl;
+    }
+    s_gbase[dgt] = __ldg(digit_base + dgt) + excl - loc;            // global slot of sorted-tile position j is s_gbase[d] + j
+#pragma unroll
+    for (int ww = 0; ww < kOsWarps; ++ww) wh[ww * kRadix + dgt] += loc;
+    __syncthreads();
+
+#pragma unroll
+    for (int r = 0; r < kOsItems; ++r) {
+        if (base + (size_t)r * 32 < n) {
+            const uint32_t d = (k[r] >> shift) & mask;
+            const uint32_t pos = mywh[d] + ((rk[r >> 1] >> (16 * (r & 1))) & 0xFFFFu);
+            s_keys[pos] = k[r]; s_vals[pos] = v[r];
+        }
+    }
+    __syncthreads();
+    for (uint32_t j = threadIdx.x; j < cnt; j += kOsThreads) {
+        const uint32_t key = s_keys[j];
+        const uint32_t dst = s_gbase[(key >> shift) & mask] + j;
+        out_keys[dst] = key; out_vals[dst] = s_vals[j];
+    }
+}
+
+int radix_passes(int key_bits) { return std::max(1, (key_bits + kRadixBits - 1) / kRadixBits); }
+
+// sorts (keys, row) by key; returns which of the double buffers holds the result (0 = a, 1 = b).
+// d_digit_hist must hold the per-pass digit counts of keys_a (k_keys_pack); d_status (zeroed by this call) has
+// passes * sort_tiles(n) * kRadix entries; d_ticket kMaxPasses entries.
+int launch_radix_sort(uint32_t* keys_a, uint32_t* keys_b, uint32_t* val_a, uint32_t* val_b, uint32_t n, int key_bits,
+                      const uint32_t* d_digit_hist, uint32_t* d_digit_base, uint32_t* d_status, uint32_t* d_ticket,
+                      cudaStream_t s) {
+    if (n == 0) return 0;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaFuncSetAttribute(k_onesweep<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kOsSmem);
+        cudaFuncSetAttribute(k_onesweep<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kOsSmem);
+        attr_set = true;
+    }
+    const int passes = radix_passes(key_bits);
+    const uint32_t n_tiles = (uint32_t)sort_tiles(n);
+    cudaMemsetAsync(d_status, 0, (size_t)passes * n_tiles * kRadix * sizeof(uint32_t), s);
+    cudaMemsetAsync(d_ticket, 0, kMaxPasses * sizeof(uint32_t), s);
+    k_digit_scan<<<1, kRadix, 0, s>>>(d_digit_hist, d_digit_base, passes); count_launch();
+    uint32_t *ki = keys_a, *ko = keys_b, *vi = val_a, *vo = val_b;
+    for (int p = 0; p < passes; ++p) {
+        const int shift = kRadixBits * p;
+        const int bits = std::min(kRadixBits, std::max(1, key_bits - shift));
+        const uint32_t mask = (1u << bits) - 1u;
+        uint32_t* st = d_status + (size_t)p * n_tiles * kRadix;
+        if (p == 0) k_onesweep<true><<<n_tiles, kOsThreads, kOsSmem, s>>>(ki, vi, n, shift, mask, d_digit_base + p * kRadix, st, d_ticket + p, ko, vo);
+        else        k_onesweep<false><<<n_tiles, kOsThreads, kOsSmem, s>>>(ki, vi, n, shift, mask, d_digit_base + p * kRadix, st, d_ticket + p, ko, vo);
+        count_launch();
+        std::swap(ki, ko); std::swap(vi, vo);
+    }
+    return passes & 1;
+}
+
+// ------------------------------------------------------------------------------------------
+// (a3) gather: sorted row order -> SoA unit vectors + ids.  One 32-byte sector per source.
+// ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
-k_gather(const double* __restrict__ ra, const double* __restrict__ dec, const int64_t* __restrict__ id,
-         const uint32_t* __restrict__ perm, uint32_t n,
+k_gather(const Rec* __restrict__ rec, const uint32_t* __restrict__ perm, uint32_t n,
          double* __restrict__ x, double* __restrict__ y, double* __restrict__ z, int64_t* __restrict__ out_id) {
     for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (size_t)gridDim.x * 256) {
-        uint32_t p = __ldg(perm + i);
-        double a = __ldg(ra + p), d = __ldg(dec + p);
-        int64_t v = id ? __ldg(id + p) : (int64_t)p;
-        double ux = 0.0, uy = 0.0, uz = 2.0;      // bad coordinate: a point no chord test can reach
-        if (coord_ok(a, d)) unit_vector(norm_ra(a), d, ux, uy, uz);
-        x[i] = ux; y[i] = uy; z[i] = uz; out_id[i] = v;
+        const double2* q = reinterpret_cast<const double2*>(rec + __ldg(perm + i));
+        const double2 a = __ldg(q), b = __ldg(q + 1);
+        x[i] = a.x; y[i] = a.y; z[i] = b.x; out_id[i] = __double_as_longlong(b.y);
     }
 }
 
-void launch_gather(const double* ra, const double* dec, const int64_t* id, const uint32_t* perm, uint32_t n,
-                   double* x, double* y, double* z, int64_t* out_id, cudaStream_t s) {
+void launch_gather(const Rec* rec, const uint32_t* perm, uint32_t n, double* x, double* y, double* z, int64_t* out_id,
+                   cudaStream_t s) {
     if (n == 0) return;
     int blocks = (int)std::min<size_t>(((size_t)n + 255) / 256, (size_t)sm_count() * 16);
-    k_gather<<<blocks, 256, 0, s>>>(ra, dec, id, perm, n, x, y, z, out_id); count_launch();
+    k_gather<<<blocks, 256, 0, s>>>(rec, perm, n, x, y, z, out_id); count_launch();
 }
 
 // ------------------------------------------------------------------------------------------
-// (a4) cell offset table: mark the first sorted row of every occupied cell, then a reverse
-// inclusive min-scan gives every (also empty) cell the first row at or after it.
+// (a4) cell offset table.  Sorted row i is the first row of every cell in (key[i-1], key[i]]; row n (one past
+// the end) closes every cell above key[n-1].  Short runs are written by the owning lane, medium runs by its
+// warp, long runs (empty sky) go to a list that k_cell_fill_big spreads over the whole grid.
 // ------------------------------------------------------------------------------------------
+constexpr uint32_t kFillLane = 4, kFillWarp = 4096;
+
 __global__ void __launch_bounds__(256)
-k_mark_heads(const uint32_t* __restrict__ keys, uint32_t n, uint32_t n_cells, uint32_t* __restrict__ cell_start) {
-    for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i <= n; i += (size_t)gridDim.x * 256) {
-        if (i == n) { cell_start[n_cells] = n; break; }
-        uint32_t k = __ldg(keys + i);
-        if (i == 0 || __ldg(keys + i - 1) != k) cell_start[k] = (uint32_t)i;
+k_cell_fill(const uint32_t* __restrict__ keys, uint32_t n, uint32_t n_cells, uint32_t* __restrict__ cell_start,
+            uint32_t* __restrict__ big, uint32_t* __restrict__ big_count, uint32_t big_cap) {
+    const int lane = threadIdx.x & 31;
+    const size_t total = (size_t)n + 1;
+    const size_t stride = (size_t)gridDim.x * 256;
+    for (size_t b = (size_t)blockIdx.x * 256 + (threadIdx.x & ~31); b < total; b += stride) {   // warp-uniform trip count
+        const size_t i = b + lane;
+        uint32_t lo = 1, hi = 0;                           // empty
+        if (i < total) {
+            hi = i < n ? __ldg(keys + i) : n_cells;
+            lo = i > 0 ? __ldg(keys + i - 1) + 1u : 0u;
+            if (i > 0 && i < n && hi + 1u == lo) { lo = 1; hi = 0; }      // same cell as the previous row
+        }
+        const uint32_t span = hi >= lo ? hi - lo + 1u : 0u;
+        if (span && span <= kFillLane) for (uint32_t c = lo; c <= hi; ++c) cell_start[c] = (uint32_t)i;
+        unsigned m = __ballot_sync(0xffffffffu, span > kFillLane);
+        while (m) {
+            const int src = __ffs(m) - 1; m &= m - 1;
+            const uint32_t l = __shfl_sync(0xffffffffu, lo, src), h = __shfl_sync(0xffffffffu, hi, src);
+            const uint32_t v = (uint32_t)(b + src);
+            if (h - l + 1u <= kFillWarp) {
+                for (uint64_t cc = (uint64_t)l + lane; cc <= h; cc += 32) cell_start[cc] = v;
+            } else if (lane == 0) {
+                uint32_t e = atomicAdd(big_count, 1u);
+                if (e < big_cap) { big[3 * e] = l; big[3 * e + 1] = h; big[3 * e + 2] = v; }
+            }
+        }
     }
 }
 
+__global__ void __launch_bounds__(256)
+k_cell_fill_big(const uint32_t* __restrict__ big, const uint32_t* __restrict__ big_count, uint32_t big_cap,
+                uint32_t* __restrict__ cell_start) {
+    const uint32_t m = min(*big_count, big_cap);
+    for (uint32_t e = 0; e < m; ++e) {
+        const uint32_t l = big[3 * e], h = big[3 * e + 1], v = big[3 * e + 2];
+        for (uint64_t c = (uint64_t)l + (size_t)blockIdx.x * 256 + threadIdx.x; c <= h; c += (uint64_t)gridDim.x * 256) cell_start[c] = v;
+    }
+}
+
+size_t cell_big_cap(size_t n_cells) { return n_cells / kFillWarp + 2; }
+
 void launch_cell_table(const uint32_t* sorted_keys, uint32_t n, uint32_t n_cells, uint32_t* cell_start,
-                       uint32_t* d_partials, cudaStream_t s) {
-    cudaMemsetAsync(cell_start, 0xFF, ((size_t)n_cells + 1) * sizeof(uint32_t), s);
+                       uint32_t* d_big /*[3*cap + 1]*/, cudaStream_t s) {
+    const uint32_t cap = (uint32_t)cell_big_cap(n_cells);
+    uint32_t* d_count = d_big + 3 * (size_t)cap;
+    cudaMemsetAsync(d_count, 0, sizeof(uint32_t), s);
     int blocks = (int)std::min<size_t>(((size_t)n + 1 + 255) / 256, (size_t)sm_count() * 16);
-    k_mark_heads<<<blocks, 256, 0, s>>>(sorted_keys, n, n_cells, cell_start); count_launch();
-    device_scan<OpMin, true, true>(cell_start, (size_t)n_cells + 1, d_partials, s);
+    k_cell_fill<<<blocks, 256, 0, s>>>(sorted_keys, n, n_cells, cell_start, d_big, d_count, cap); count_launch();
+    k_cell_fill_big<<<sm_count() * 4, 256, 0, s>>>(d_big, d_count, cap, cell_start); count_launch();
+}
+
+// ------------------------------------------------------------------------------------------
+// (a4) tile descriptors: tile = up to kTile consecutive sorted rows of ONE zone (the role of the paper's
+// calculation blocks: there cut to fit the N^2 result matrix, here to fit one CTA).
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(1024)
+k_zone_tiles(const uint32_t* __restrict__ cell_start, const uint32_t* __restrict__ cell_base, uint32_t n_zones,
+             uint32_t* __restrict__ tile_first /*[n_zones + 1]*/, uint32_t* __restrict__ n_tiles) {
+    __shared__ uint32_t sm[33];
+    uint32_t carry = 0;
+    for (uint32_t b = 0; b < n_zones; b += 1024) {
+        const uint32_t z = b + threadIdx.x;
+        uint32_t t = 0;
+        if (z < n_zones) {
+            const uint32_t cnt = __ldg(cell_start + __ldg(cell_base + z + 1)) - __ldg(cell_start + __ldg(cell_base + z));
+            t = (cnt + kTile - 1) / kTile;
+        }
+        uint32_t tot;
+        const uint32_t inc = block_scan_incl(t, &tot, sm);
+        if (z < n_zones) tile_first[z] = carry + inc - t;
+        carry += tot;
+    }
+    if (threadIdx.x == 0) { tile_first[n_zones] = carry; *n_tiles = carry; }
+}
+
+__global__ void __launch_bounds__(256)
+k_tile_desc(const uint32_t* __restrict__ tile_first, uint32_t n_zones, const uint32_t* __restrict__ cell_start,
+            const uint32_t* __restrict__ cell_base, const uint32_t* __restrict__ keys, TileDesc* __restrict__ tiles) {
+    const uint32_t nt = __ldg(tile_first + n_zones);
+    for (uint32_t t = blockIdx.x * 256 + threadIdx.x; t < nt; t += gridDim.x * 256) {
+        uint32_t lo = 0, hi = n_zones;                // largest z with tile_first[z] <= t
+        while (hi - lo > 1) { uint32_t mid = (lo + hi) >> 1; if (__ldg(tile_first + mid) <= t) lo = mid; else hi = mid; }
+        const uint32_t z = lo, cb = __ldg(cell_base + z);
+        const uint32_t zs = __ldg(cell_start + cb), ze = __ldg(cell_start + __ldg(cell_base + z + 1));
+        const uint32_t s0 = zs + (t - __ldg(tile_first + z)) * kTile;
+        const uint32_t m = min((uint32_t)kTile, ze - s0);
+        TileDesc d;
+        d.first = s0; d.count = m; d.zone = z;
+        d.k_first = __ldg(keys + s0) - cb; d.k_last = __ldg(keys + s0 + m - 1) - cb;
+        d.pad0 = d.pad1 = d.pad2 = 0;
+        tiles[t] = d;
+    }
+}
+
+void launch_tiles(const uint32_t* cell_start, const uint32_t* cell_base, uint32_t n_zones, const uint32_t* sorted_keys,
+                  uint32_t tile_cap, uint32_t* d_tile_first, TileDesc* tiles, uint32_t* d_n_tiles, cudaStream_t s) {
+    k_zone_tiles<<<1, 1024, 0, s>>>(cell_start, cell_base, n_zones, d_tile_first, d_n_tiles); count_launch();
+    int blocks = (int)std::min<size_t>(((size_t)tile_cap + 255) / 256, (size_t)sm_count() * 8);
+    k_tile_desc<<<std::max(blocks, 1), 256, 0, s>>>(d_tile_first, n_zones, cell_start, cell_base, sorted_keys, tiles); count_launch();
 }
 
 }  // namespace hlc2

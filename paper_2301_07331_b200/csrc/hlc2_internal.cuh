@@ -10,13 +10,19 @@ namespace hlc2 {
 
 constexpr int kRaBins = 4096;                 // coarse RA histogram of the extent pass
 constexpr double kRaBinDeg = 360.0 / kRaBins; // 0.087890625, exact
-constexpr uint32_t kMaxN = 0xFFFFFFFEu;
+constexpr uint32_t kMaxN = (1u << 30) - 1;    // the radix sort's chained scan keeps 2 flag bits beside a 30-bit count
+
+constexpr int kRadixBits = 9;                 // LSD radix sort digit
+constexpr int kRadix = 1 << kRadixBits;
+constexpr int kMaxPasses = 4;                 // 32-bit keys
+constexpr int kTile = 256;                    // sources per match tile (= threads of the match CTA)
 
 // ---- grid as the kernels see it (passed by value) ----------------------------------------
 struct GridView {
     const int32_t* n_ra;        // [n_zones] RA cells per zone
     const uint32_t* cell_base;  // [n_zones + 1] first cell key of each zone
     double dec_lo;              // south edge of zone 0 (deg)
+    double h;                   // zone height (deg)
     double inv_h;               // 1 / zone height (1/deg)
     double ra0;                 // west edge of the RA box (deg)
     double span;                // RA extent of the box (deg), 360 = full ring
@@ -26,13 +32,25 @@ struct GridView {
     uint32_t n_cells;
 };
 
+// tile of the cell-sorted catalogue: rows [first, first + count) all lie in `zone`, in its cells k_first..k_last
+struct TileDesc {
+    uint32_t first, count, zone, k_first, k_last, pad0, pad1, pad2;
+};
+static_assert(sizeof(TileDesc) == 32, "TileDesc is read as two 16-byte words");
+
 struct IndexView {
     const double* x; const double* y; const double* z;   // [n] unit vectors, cell order
     const int64_t* id;                                    // [n]
     const uint32_t* cell_start;                           // [n_cells + 1]
+    const TileDesc* tiles;                                // [*n_tiles]
+    const uint32_t* n_tiles;                              // device scalar
     GridView g;
     uint32_t n;
+    uint32_t tile_cap;                                    // host-side upper bound of *n_tiles
 };
+
+// packed per-source record in INPUT order, written by the key pass and read (one sector) by the gather
+struct __align__(32) Rec { double x, y, z; long long id; };
 
 // extent statistics written by the stats pass
 struct Stats {
@@ -44,21 +62,28 @@ struct Stats {
 };
 
 // ---- launchers (hlc2_build.cu, hlc2_match.cu) --------------------------------------------
+int sm_count();
 void launch_stats(const double* ra, const double* dec, uint32_t n, Stats* d_stats, cudaStream_t s);
-void launch_keys(const double* ra, const double* dec, uint32_t n, GridView g, uint32_t* keys, cudaStream_t s);
+void launch_keys_pack(const double* ra, const double* dec, const int64_t* id, uint32_t n, GridView g, int passes,
+                      uint32_t* keys, Rec* rec, uint32_t* digit_hist, cudaStream_t s);
+int  radix_passes(int key_bits);
+size_t sort_tiles(uint32_t n);
 // sorts (keys, row) by key; returns which of the double buffers holds the result (0 = a, 1 = b)
-int  launch_radix_sort(uint32_t* keys_a, uint32_t* keys_b, uint32_t* val_a, uint32_t* val_b, uint32_t n,
-                       int key_bits, uint32_t* d_counts, size_t counts_entries, uint32_t* d_partials, cudaStream_t s);
-void launch_gather(const double* ra, const double* dec, const int64_t* id, const uint32_t* perm, uint32_t n,
-                   double* x, double* y, double* z, int64_t* out_id, cudaStream_t s);
+int  launch_radix_sort(uint32_t* keys_a, uint32_t* keys_b, uint32_t* val_a, uint32_t* val_b, uint32_t n, int key_bits,
+                       const uint32_t* d_digit_hist, uint32_t* d_digit_base, uint32_t* d_status, uint32_t* d_ticket,
+                       cudaStream_t s);
+void launch_gather(const Rec* rec, const uint32_t* perm, uint32_t n, double* x, double* y, double* z, int64_t* out_id,
+                   cudaStream_t s);
+size_t cell_big_cap(size_t n_cells);
 void launch_cell_table(const uint32_t* sorted_keys, uint32_t n, uint32_t n_cells, uint32_t* cell_start,
-                       uint32_t* d_partials, cudaStream_t s);
-size_t sort_counts_entries(uint32_t n);      // entries of the digit-count array for n keys
-size_t scan_partials_entries(size_t m);      // entries of the partial-sum array for a scan over m entries
+                       uint32_t* d_big, cudaStream_t s);
+void launch_tiles(const uint32_t* cell_start, const uint32_t* cell_base, uint32_t n_zones, const uint32_t* sorted_keys,
+                  uint32_t tile_cap, uint32_t* d_tile_first, TileDesc* tiles, uint32_t* d_n_tiles, cudaStream_t s);
 
+size_t match_temp_bytes(const IndexView& A, const IndexView& B);
 void launch_match(const IndexView& A, const IndexView& B, double radius_arcsec, int mode,
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
-                  unsigned long long* d_count, cudaStream_t s);
+                  unsigned long long* d_count, void* d_temp, cudaStream_t s);
 
 void count_launch(int k = 1);
 

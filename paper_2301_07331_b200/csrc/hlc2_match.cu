@@ -130,9 +130,12 @@ k_match(IndexView A, IndexView B, MatchArgs p) {
     }
 }
 
+size_t match_temp_bytes(const IndexView&, const IndexView&) { return 0; }
+
 void launch_match(const IndexView& A, const IndexView& B, double radius_arcsec, int mode,
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
-                  unsigned long long* d_count, cudaStream_t s) {
+                  unsigned long long* d_count, void* d_temp, cudaStream_t s) {
+    (void)d_temp;
     if (A.n == 0) return;
     MatchArgs p;
     long double r_rad = (long double)radius_arcsec * (3.141592653589793238462643383279502884L / 648000.0L);
