@@ -38,7 +38,7 @@ struct HostGrid {
 };
 
 struct Layout {           // byte offsets inside the index buffer
-    size_t x, y, z, id, key, cell_start, n_ra, cell_base, tiles, n_tiles, stats, total;
+    size_t x, y, z, id, pos, key, cell_start, n_ra, cell_base, tiles, n_tiles, stats, total;
     size_t cap_cells, cap_zones, cap_tiles, n_pad;
 };
 struct TempLayout { size_t key_b, perm_a, perm_b, rec, digit_hist, digit_base, ticket, status, big, tile_first, total; };
@@ -102,6 +102,7 @@ static Layout make_layout(int64_t n, const hlc2_opts& o) {
     L.y = off; off += align_up(L.n_pad * 8);
     L.z = off; off += align_up(L.n_pad * 8);
     L.id = off; off += align_up(L.n_pad * 8);
+    L.pos = off; off += align_up(L.n_pad * 8);
     L.key = off; off += align_up(L.n_pad * 4);
     L.cell_start = off; off += align_up((L.cap_cells + 1) * 4 + 64);   // slack: bulk copies round up to 16 bytes
     L.n_ra = off; off += align_up(L.cap_zones * 4);
@@ -205,6 +206,7 @@ static IndexView index_view(const hlc2_index* ix) {
     IndexView v;
     v.x = (const double*)(ix->d_buf + ix->lay.x); v.y = (const double*)(ix->d_buf + ix->lay.y);
     v.z = (const double*)(ix->d_buf + ix->lay.z); v.id = (const int64_t*)(ix->d_buf + ix->lay.id);
+    v.pos = (const float2*)(ix->d_buf + ix->lay.pos);
     v.cell_start = (const uint32_t*)(ix->d_buf + ix->lay.cell_start);
     v.tiles = (const TileDesc*)(ix->d_buf + ix->lay.tiles); v.n_tiles = (const uint32_t*)(ix->d_buf + ix->lay.n_tiles);
     v.g = grid_view(ix); v.n = (uint32_t)ix->n;
@@ -301,7 +303,7 @@ int hlc2_build_index(const double* d_ra, const double* d_dec, const int64_t* d_i
     int where = launch_radix_sort(ka, kb, pa, pb, nn, key_bits, digit_hist, (uint32_t*)(tmp + T.digit_base),
                                   (uint32_t*)(tmp + T.status), (uint32_t*)(tmp + T.ticket), s);
     const uint32_t* perm = where ? pb : pa;
-    launch_gather(rec, perm, nn, (double*)(buf + L.x), (double*)(buf + L.y), (double*)(buf + L.z), (int64_t*)(buf + L.id), s);
+    launch_gather(rec, perm, nn, (double*)(buf + L.x), (double*)(buf + L.y), (double*)(buf + L.z), (int64_t*)(buf + L.id), (float2*)(buf + L.pos), s);
     launch_cell_table(key_idx, nn, n_cells, (uint32_t*)(buf + L.cell_start), (uint32_t*)(tmp + T.big), s);
     launch_tiles((const uint32_t*)(buf + L.cell_start), gv.cell_base, (uint32_t)g.n_zones, key_idx,
                  (uint32_t)((size_t)n / kTile + (size_t)g.n_zones + 1), (uint32_t*)(tmp + T.tile_first),

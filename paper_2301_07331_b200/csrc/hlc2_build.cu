@@ -312,19 +312,28 @@ int launch_radix_sort(uint32_t* keys_a, uint32_t* keys_b, uint32_t* val_a, uint3
 // ------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)
 k_gather(const Rec* __restrict__ rec, const uint32_t* __restrict__ perm, uint32_t n,
-         double* __restrict__ x, double* __restrict__ y, double* __restrict__ z, int64_t* __restrict__ out_id) {
+         double* __restrict__ x, double* __restrict__ y, double* __restrict__ z, int64_t* __restrict__ out_id,
+         float2* __restrict__ pos) {
     for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (size_t)gridDim.x * 256) {
         const double2* q = reinterpret_cast<const double2*>(rec + __ldg(perm + i));
         const double2 a = __ldg(q), b = __ldg(q + 1);
         x[i] = a.x; y[i] = a.y; z[i] = b.x; out_id[i] = __double_as_longlong(b.y);
+        // fp32 (ra, dec) estimate of the sorted row: the match kernel locates its search window from it
+        // (padded by the error bound of exactly this chain); this kernel waits on
+        // scattered sectors, so the two atan2f are free here and are paid once per build, not per match
+        const float fx = (float)a.x, fy = (float)a.y, fz = (float)b.x;
+        const float rxy = sqrtf(fx * fx + fy * fy);
+        float ra_f = atan2f(fy, fx) * 57.29577951f;
+        if (ra_f < 0.0f) ra_f += 360.0f;
+        pos[i] = make_float2(ra_f, atan2f(fz, rxy) * 57.29577951f);
     }
 }
 
 void launch_gather(const Rec* rec, const uint32_t* perm, uint32_t n, double* x, double* y, double* z, int64_t* out_id,
-                   cudaStream_t s) {
+                   float2* pos, cudaStream_t s) {
     if (n == 0) return;
     int blocks = (int)std::min<size_t>(((size_t)n + 255) / 256, (size_t)sm_count() * 16);
-    k_gather<<<blocks, 256, 0, s>>>(rec, perm, n, x, y, z, out_id); count_launch();
+    k_gather<<<blocks, 256, 0, s>>>(rec, perm, n, x, y, z, out_id, pos); count_launch();
 }
 
 // ------------------------------------------------------------------------------------------

@@ -24,9 +24,8 @@ __device__ __forceinline__ bool coord_ok(double ra, double dec) {
 
 // zone of a declination (deg); monotone non-decreasing in dec
 __device__ __forceinline__ int zone_of(const GridView& g, double dec) {
-    double f = floor((dec - g.dec_lo) * g.inv_h);
-    f = fmin(fmax(f, 0.0), (double)(g.n_zones - 1));
-    return (int)f;
+    const int z = __double2int_rd((dec - g.dec_lo) * g.inv_h);      // floor, saturating; clamps are integer ops
+    return min(max(z, 0), g.n_zones - 1);
 }
 
 // box-relative RA coordinate of a normalised RA: u in [0, 360]
@@ -38,9 +37,8 @@ __device__ __forceinline__ double box_u(const GridView& g, double ra_norm) {
 
 // RA cell of box coordinate u (u >= 0) in a zone with n cells; monotone non-decreasing in u
 __device__ __forceinline__ int cell_of_u(const GridView& g, double u, int n) {
-    double f = floor((u * g.inv_span) * (double)n);
-    f = fmin(fmax(f, 0.0), (double)(n - 1));
-    return (int)f;
+    const int k = __double2int_rd((u * g.inv_span) * (double)n);
+    return min(max(k, 0), n - 1);
 }
 
 // order-preserving map fp64 -> uint64 (for atomicMin / atomicMax on doubles)

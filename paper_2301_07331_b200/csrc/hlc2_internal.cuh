@@ -41,6 +41,7 @@ static_assert(sizeof(TileDesc) == 32, "TileDesc is read as two 16-byte words");
 struct IndexView {
     const double* x; const double* y; const double* z;   // [n] unit vectors, cell order
     const int64_t* id;                                    // [n]
+    const float2* pos;                                    // [n] fp32 (ra, dec) estimate in degrees: locates windows, never decides
     const uint32_t* cell_start;                           // [n_cells + 1]
     const TileDesc* tiles;                                // [*n_tiles]
     const uint32_t* n_tiles;                              // device scalar
@@ -73,7 +74,7 @@ int  launch_radix_sort(uint32_t* keys_a, uint32_t* keys_b, uint32_t* val_a, uint
                        const uint32_t* d_digit_hist, uint32_t* d_digit_base, uint32_t* d_status, uint32_t* d_ticket,
                        cudaStream_t s);
 void launch_gather(const Rec* rec, const uint32_t* perm, uint32_t n, double* x, double* y, double* z, int64_t* out_id,
-                   cudaStream_t s);
+                   float2* pos, cudaStream_t s);
 size_t cell_big_cap(size_t n_cells);
 void launch_cell_table(const uint32_t* sorted_keys, uint32_t n, uint32_t n_cells, uint32_t* cell_start,
                        uint32_t* d_big, cudaStream_t s);
