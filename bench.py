@@ -206,7 +206,7 @@ def main():
         if marks is not None: marks[1].record()
         ib = P.hlc2_build_index(devB[0], devB[1], devB[2], opts=opts_b, temp=temp, buf=buf_b)
         if marks is not None: marks[2].record()
-        P.hlc2_crossmatch(ia, ib, r, mode, out_a, out_b, out_s, cnt)
+        P.hlc2_crossmatch(ia, ib, r, mode, out_a, out_b, out_s, cnt, temp=temp)
         if marks is not None: marks[3].record()
         return ia, ib
 

@@ -215,6 +215,12 @@ def hlc2_crossmatch(A: Index, B: Index, radius_arcsec: float, mode: int, out_ida
     Asynchronous on `stream`; read `count` after synchronising."""
     cap = int(out_ida.shape[0])
     assert out_idb.shape[0] == cap and out_sep.shape[0] == cap
+    need = hlc2_crossmatch_sizes(A, B)
+    if need and (temp is None or temp.numel() < need):
+        torch = _torch()
+        temp = torch.empty(need, dtype=torch.uint8, device=A.buf.device)
+        # the stream still owns the scratch until the enqueued work drains
+        temp.record_stream(torch.cuda.current_stream() if stream is None else stream)
     rc = lib().hlc2_crossmatch(A.handle, B.handle, float(radius_arcsec), int(mode), out_ida.data_ptr(), out_idb.data_ptr(),
                                out_sep.data_ptr(), cap, count.data_ptr(), temp.data_ptr() if temp is not None else None,
                                temp.numel() if temp is not None else 0, _stream_ptr(stream))
