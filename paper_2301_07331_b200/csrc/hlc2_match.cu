@@ -34,13 +34,29 @@ namespace hlc2 {
 
 constexpr int kCW = kTile / 32;              // consumer warps (one lane per A row of the tile)
 constexpr int kMatchThreads = kTile + 32;    // + the producer warp
-constexpr int kStages = 3;
-constexpr int kSegs = 4;                     // zone segments per job
-constexpr int kBCap = 448;                   // staged B rows per job, all segments, after 16-byte alignment
-constexpr int kCsCap = 512;                  // staged cell_start entries per job, after alignment
-constexpr int kQCap = 96;                    // rows in a warp's hit queue
-constexpr int kQFlush = 64;                  // flushed as soon as this many are queued (<= 63 + 32 < kQCap)
+#ifndef HLC2_STAGES
+#define HLC2_STAGES 2
+#endif
+#ifndef HLC2_BCAP
+#define HLC2_BCAP 320
+#endif
+#ifndef HLC2_CSCAP
+#define HLC2_CSCAP 512
+#endif
+#ifndef HLC2_QCAP
+#define HLC2_QCAP 64
+#endif
+#ifndef HLC2_CTAS
+#define HLC2_CTAS 5
+#endif
+constexpr int kStages = HLC2_STAGES;
+constexpr int kSegs = 3;                     // window pieces per job
+constexpr int kBCap = HLC2_BCAP;             // staged B rows per job, all pieces, after 16-byte alignment
+constexpr int kCsCap = HLC2_CSCAP;           // staged cell_start entries per job, after alignment
+constexpr int kQCap = HLC2_QCAP;             // rows in a warp's hit queue
+constexpr int kQFlush = kQCap - 32;          // flushed as soon as this many are queued (at most kQFlush - 1 + 32 are ever held)
 constexpr int kAPad = kTile + 2;             // A tile rows after alignment to 16 bytes
+constexpr int kMaxZones = 8;                 // tiles whose window spans more zones of B's grid take the general path
 constexpr double kRad2Arcsec = 206264.80624709636;   // 648000 / pi
 constexpr unsigned kFull = 0xffffffffu;
 
@@ -49,12 +65,20 @@ constexpr double kEpsRaDeg = 2.5e-4;
 constexpr double kEpsDecDeg = 1.5e-4;
 constexpr double kTinyDeg = 1e-9;            // fp64 slop on cell / zone edges in the planner
 
-constexpr uint32_t kJobDirect = 1u << 8;
+// job flags (bits 0-3: number of pieces)
+constexpr uint32_t kJobDirect = 1u << 8;     // general per-lane path from global memory
+constexpr uint32_t kJobRing = 1u << 9;       // every row takes all cells of every piece (polar tiles)
+constexpr uint32_t kJobWrap = 1u << 10;      // window touches u = 0 / 360: rows re-centre their RA on each piece
+constexpr uint32_t kJobFirst = 1u << 11;     // first / last job of its A tile (nearest mode carries the best across jobs)
+constexpr uint32_t kJobLast = 1u << 12;
+constexpr uint32_t kJobEnd = 1u << 13;       // producer -> consumers: no more work
 
-// 96-byte job record (24 words), one per A tile, written by k_plan
-struct JobSeg { uint32_t row_lo, cs_lo; int32_t k_lo, n_ra; uint32_t nk_nrows; };   // n_k | n_rows << 16
-struct Job { uint32_t a_first, a_count; int32_t z_lo; uint32_t flags; JobSeg seg[kSegs]; };
-static_assert(sizeof(Job) == 96, "the producer reads a job as 24 words");
+// 128-byte job record (32 words).  jobs[t] is the first job of A tile t; further jobs of a tile (windows that do
+// not fit one stage: the paper's calculation blocks, L253-257, cut to fit shared memory) are chained by `next`.
+// A piece = cells [k_lo, k_lo + nk) of one zone of B's grid restricted to B rows [row_lo, row_lo + n_rows).
+struct JobSeg { int32_t zone, k_lo; uint32_t nk, row_lo, n_rows; int32_t n_ra; uint32_t cs_lo; float centre; };
+struct Job { uint32_t a_first, a_count, flags, next; JobSeg seg[kSegs]; uint32_t pad[4]; };
+static_assert(sizeof(JobSeg) == 32 && sizeof(Job) == 128, "the producer reads a job as 32 words");
 
 struct MatchArgs {
     double thr2;          // 4 sin^2(r/2)
@@ -64,11 +88,13 @@ struct MatchArgs {
     int64_t* out_ida; int64_t* out_idb; double* out_sep;
     unsigned long long capacity;
     unsigned long long* count;
-    const Job* jobs;
+    Job* jobs;            // [tile_cap] first jobs, then [pool_cap] chained jobs
+    uint32_t* pool_count;
+    uint32_t tile_cap, pool_cap;
 };
 
-struct SegDesc { double n_d; int32_t k_lo, k_hi, cdelta; uint32_t rdelta, n_rows, pad; };
-struct StageDesc { uint32_t a_first, a_count, a_off, flags; int32_t nseg, z_lo; uint32_t pad[2]; SegDesc seg[kSegs]; };
+struct SegDesc { double n_d; double centre; int32_t zone, k_lo, k_hi, cdelta; uint32_t rdelta, row_lo, row_hi, pad; };
+struct StageDesc { uint32_t a_count, a_off, flags; int32_t nseg; SegDesc seg[kSegs]; };
 
 struct __align__(16) Stage {
     double ax[kAPad], ay[kAPad], az[kAPad];
@@ -107,6 +133,17 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity
                      : "=r"(done) : "r"(a), "r"(parity) : "memory");
     } while (!done);
 }
+// the producer runs ahead and mostly waits for a free stage: back off between polls so that it does not eat issue slots
+__device__ __forceinline__ void mbar_wait_backoff(unsigned long long* b, unsigned parity) {
+    const uint32_t a = smem_u32(b);
+    unsigned done;
+    for (;;) {
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(done) : "r"(a), "r"(parity) : "memory");
+        if (done) break;
+        __nanosleep(256);
+    }
+}
 // global -> shared bulk copy, completion counted in bytes on an mbarrier; 16-byte aligned src, dst and size
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* b) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -124,81 +161,138 @@ __device__ __forceinline__ double sep_from_chord2(double c2) {
 }
 
 // ------------------------------------------------------------------------------------------------------
-// k_plan: one job per A tile
+// k_plan: the jobs of every A tile
 // ------------------------------------------------------------------------------------------------------
+struct PlanState {
+    uint32_t w[32];            // the job being assembled
+    uint32_t slot;             // where it will be written
+    uint32_t rows_used, cs_used;
+    int nseg;
+    bool first, overflow;
+};
+
+__device__ __forceinline__ void plan_store(Job* jobs, uint32_t slot, const uint32_t* w) {
+    uint4* o = reinterpret_cast<uint4*>(jobs + slot);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) o[i] = make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
+}
+
+// write the assembled job; unless it is the tile's last one, take a pool slot for its successor
+__device__ __noinline__ void plan_close(PlanState& st, const MatchArgs& p, uint32_t common, bool last) {
+    uint32_t next = 0;
+    if (!last) {
+        const uint32_t idx = atomicAdd(p.pool_count, 1u);
+        if (idx >= p.pool_cap) { st.overflow = true; return; }
+        next = p.tile_cap + idx;
+    }
+    st.w[2] = (uint32_t)st.nseg | common | (st.first ? kJobFirst : 0u) | (last ? kJobLast : 0u);
+    st.w[3] = next;
+    plan_store(p.jobs, st.slot, st.w);
+    st.slot = next; st.first = false; st.nseg = 0; st.rows_used = 0; st.cs_used = 0;
+#pragma unroll
+    for (int i = 4; i < 32; ++i) st.w[i] = 0;
+}
+
+// cells [ka, kb] of zone z: cut into pieces that fit what is left of the current job, opening new jobs as needed
+__device__ __noinline__ void plan_piece(PlanState& st, const MatchArgs& p, const uint32_t* __restrict__ cs, uint32_t common,
+                                        int z, int n, uint32_t cb, int ka, int kb, float centre) {
+    uint32_t ra = __ldg(cs + cb + (uint32_t)ka);
+    const uint32_t rb = __ldg(cs + cb + (uint32_t)kb + 1u);
+    while (ra < rb && !st.overflow) {
+        if (st.nseg == kSegs || st.rows_used + 4u > (uint32_t)kBCap || st.cs_used + 12u > (uint32_t)kCsCap) {
+            plan_close(st, p, common, false);
+            if (st.overflow) return;
+        }
+        const uint32_t max_rows = (uint32_t)kBCap - st.rows_used - 2u, max_cells = (uint32_t)kCsCap - st.cs_used - 8u;
+        int ke = (int)min((long long)kb, (long long)ka + (long long)max_cells - 1);
+        uint32_t re = ke == kb ? rb : __ldg(cs + cb + (uint32_t)ke + 1u);
+        if (re - ra > max_rows) {
+            re = ra + max_rows;
+            int lo = ka, hi = ke;                           // largest k with cs[k] < re: the cell holding row re - 1
+            while (lo < hi) {
+                const int mid = (int)(((long long)lo + hi + 1) >> 1);
+                if (__ldg(cs + cb + (uint32_t)mid) < re) lo = mid; else hi = mid - 1;
+            }
+            ke = lo;
+        }
+        uint32_t* s = st.w + 4 + 8 * st.nseg;
+        s[0] = (uint32_t)z; s[1] = (uint32_t)ka; s[2] = (uint32_t)(ke - ka + 1); s[3] = ra; s[4] = re - ra;
+        s[5] = (uint32_t)n; s[6] = cb + (uint32_t)ka; s[7] = __float_as_uint(centre);
+        st.rows_used += ((re + 1u) & ~1u) - (ra & ~1u);
+        st.cs_used += ((cb + (uint32_t)ke + 2u + 3u) & ~3u) - ((cb + (uint32_t)ka) & ~3u);
+        ++st.nseg;
+        if (re >= rb) break;
+        ra = re;
+        ka = (ke < kb && __ldg(cs + cb + (uint32_t)ke + 1u) <= re) ? ke + 1 : ke;     // the cell holding row `re`
+    }
+}
+
 __global__ void __launch_bounds__(128)
-k_plan(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B, const __grid_constant__ MatchArgs p,
-       Job* __restrict__ jobs) {
+k_plan(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B, const __grid_constant__ MatchArgs p) {
     const uint32_t nt = __ldg(A.n_tiles);
     const GridView& ga = A.g;
     const GridView& gb = B.g;
     for (uint32_t t = blockIdx.x * 128 + threadIdx.x; t < nt; t += gridDim.x * 128) {
         const uint4 t0 = __ldg(reinterpret_cast<const uint4*>(A.tiles + t));        // first, count, zone, k_first
         const uint4 t1 = __ldg(reinterpret_cast<const uint4*>(A.tiles + t) + 1);    // k_last
-        uint32_t w[24];
+        PlanState st;
 #pragma unroll
-        for (int i = 0; i < 24; ++i) w[i] = 0;
-        w[0] = t0.x; w[1] = t0.y;
+        for (int i = 0; i < 32; ++i) st.w[i] = 0;
+        st.w[0] = t0.x; st.w[1] = t0.y;
+        st.slot = t; st.rows_used = 0; st.cs_used = 0; st.nseg = 0; st.first = true; st.overflow = false;
         const int za = (int)t0.z;
         // declination and RA bounds of the tile's rows: the edges of its zone and of its first / last cell in
         // A's grid (rows were filed by the same floor expressions; kTinyDeg covers their rounding)
         const double dlo = za == 0 ? ga.dec_min : fmax(ga.dec_min, ga.dec_lo + (double)za * ga.h - kTinyDeg);
         const double dhi = za == ga.n_zones - 1 ? ga.dec_max : fmin(ga.dec_max, ga.dec_lo + (double)(za + 1) * ga.h + kTinyDeg);
         const double qlo = dlo - p.r_deg - kTinyDeg, qhi = dhi + p.r_deg + kTinyDeg;
-        bool empty = qhi < gb.dec_min || qlo > gb.dec_max || t0.y == 0;
+        const bool empty = qhi < gb.dec_min || qlo > gb.dec_max || t0.y == 0;
         bool direct = false;
+        uint32_t common = 0;
         if (!empty) {
             const int zb0 = zone_of(gb, qlo), zb1 = zone_of(gb, qhi);
-            const int nseg = zb1 - zb0 + 1;
-            if (nseg > kSegs) direct = true;
+            if (zb1 - zb0 + 1 > kMaxZones) direct = true;
             const double cw = ga.span / (double)__ldg(ga.n_ra + za);
             const double ua_lo = (double)t0.w * cw - kTinyDeg, ua_hi = (double)(t1.x + 1u) * cw + kTinyDeg;
             // RA half-window of the most poleward row: sin(dRA) = sin r / cos dec; the rows bound asin(s) by
             // 1.011 s (s < 0.25) from their own fp32 cos dec; the extra 1.001 and kEpsRaDeg keep W above all of them
             const double dabs = fmin(90.0, fmax(fabs(dlo), fabs(dhi)));
             const double s = (double)p.sin_r_up / fmax(cos(dabs * 0.017453292519943295), 1e-300);
-            if (!(s < 0.2)) direct = true;
             const double W = s * (1.011 * 57.29577951308232 * 1.001) + 2.0 * kEpsRaDeg;
             double ub = (ga.ra0 + ua_lo) - gb.ra0;
             ub -= 360.0 * floor(ub * (1.0 / 360.0));
             if (!(ub >= 0.0 && ub < 360.0)) ub = 0.0;
-            const double lo = ub - W, hi = ub + (ua_hi - ua_lo) + W;
-            // a window that comes within the estimate's error of u = 0 / 360 could see a row's estimate wrap
-            if (!(lo >= 2.0 * kEpsRaDeg) || !(hi + 2.0 * kEpsRaDeg < 360.0)) direct = true;
-            if (!direct && lo > gb.span + 2.0 * kEpsRaDeg) empty = true;      // beyond B's RA box
-            if (!direct && !empty) {
-                uint32_t rows_tot = 0, cs_tot = 0;
-                w[2] = (uint32_t)zb0;
-#pragma unroll
-                for (int sg = 0; sg < kSegs; ++sg) {
-                    if (sg < nseg) {
-                        const int z = zb0 + sg, n = __ldg(gb.n_ra + z);
+            const double L = ub - W, H = ub + (ua_hi - ua_lo) + W;           // the tile's RA window in B's box frame
+            const bool ring = !(s < 0.2) || !(H - L < 300.0);
+            // up to two RA intervals inside [0, span]: the window itself and its image through u = 0 / 360
+            double ilo[2], ihi[2]; float ctr[2]; int ni = 0;
+            if (ring) { common |= kJobRing; ilo[0] = 0.0; ihi[0] = gb.span; ctr[0] = 0.0f; ni = 1; }
+            else {
+                if (!(L >= 2.0 * kEpsRaDeg) || !(H + 2.0 * kEpsRaDeg < 360.0)) common |= kJobWrap;
+                const float c = (float)(0.5 * (L + H));
+                if (H >= 0.0 && L <= gb.span) { ilo[ni] = fmax(L, 0.0); ihi[ni] = fmin(H, gb.span); ctr[ni] = c; ++ni; }
+                if (L < 0.0 && L + 360.0 <= gb.span) { ilo[ni] = L + 360.0; ihi[ni] = fmin(H + 360.0, gb.span); ctr[ni] = c + 360.0f; ++ni; }
+                else if (H >= 360.0) { ilo[ni] = fmax(L - 360.0, 0.0); ihi[ni] = fmin(H - 360.0, gb.span); ctr[ni] = c - 360.0f; ++ni; }
+            }
+            if (!direct) {
+                for (int i = 0; i < ni && !st.overflow; ++i)
+                    for (int z = zb0; z <= zb1 && !st.overflow; ++z) {
+                        const int n = __ldg(gb.n_ra + z);
                         const uint32_t cb = __ldg(gb.cell_base + z);
-                        const int k0 = cell_of_u(gb, lo, n), k1 = cell_of_u(gb, hi, n);
-                        const uint32_t r0 = __ldg(B.cell_start + cb + (uint32_t)k0), r1 = __ldg(B.cell_start + cb + (uint32_t)k1 + 1u);
-                        const uint32_t nk = (uint32_t)(k1 - k0 + 1), nr = r1 - r0, c0 = cb + (uint32_t)k0;
-                        if (nr) {
-                            rows_tot += ((r1 + 1u) & ~1u) - (r0 & ~1u);
-                            cs_tot += ((c0 + nk + 1u + 3u) & ~3u) - (c0 & ~3u);
-                        }
-                        if (nk > 0xFFFFu || nr > 0xFFFFu) direct = true;
-                        w[4 + 5 * sg] = r0; w[5 + 5 * sg] = c0; w[6 + 5 * sg] = (uint32_t)k0; w[7 + 5 * sg] = (uint32_t)n;
-                        w[8 + 5 * sg] = (nk & 0xFFFFu) | (nr << 16);
+                        const int k0 = ring ? 0 : cell_of_u(gb, ilo[i], n), k1 = ring ? n - 1 : cell_of_u(gb, ihi[i], n);
+                        plan_piece(st, p, B.cell_start, common, z, n, cb, k0, k1, ctr[i]);
                     }
-                }
-                if (rows_tot > (uint32_t)kBCap || cs_tot > (uint32_t)kCsCap) direct = true;
-                if (rows_tot == 0) empty = true;
-                w[3] = (uint32_t)nseg;
+                if (st.overflow) direct = true;
             }
         }
-        if (direct || empty) {
+        if (direct) {                       // general path: one job, no pieces (rewrites the tile's first job)
 #pragma unroll
-            for (int i = 2; i < 24; ++i) w[i] = 0;
-            if (direct && !empty) w[3] = kJobDirect;
+            for (int i = 4; i < 32; ++i) st.w[i] = 0;
+            st.w[2] = kJobDirect | kJobFirst | kJobLast; st.w[3] = 0;
+            plan_store(p.jobs, t, st.w);
+        } else {
+            plan_close(st, p, common, true);        // a tile without pieces ends up as one empty job
         }
-        uint4* o = reinterpret_cast<uint4*>(jobs + t);
-#pragma unroll
-        for (int i = 0; i < 6; ++i) o[i] = make_uint4(w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
     }
 }
 
@@ -340,7 +434,7 @@ __device__ __forceinline__ void scan_staged(const Stage& st, const MatchArgs& p,
 // k_match
 // ------------------------------------------------------------------------------------------------------
 template <int MODE>
-__global__ void __launch_bounds__(kMatchThreads, 3)
+__global__ void __launch_bounds__(kMatchThreads, HLC2_CTAS)
 k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B, const __grid_constant__ MatchArgs p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     MatchSmem& sm = *reinterpret_cast<MatchSmem*>(smem_raw);
@@ -351,28 +445,35 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
     }
     if (threadIdx.x < kStages) { Stage& st = sm.st[threadIdx.x]; st.bx[kBCap] = 0.0; st.by[kBCap] = 0.0; st.bz[kBCap] = 2.0; }
     __syncthreads();
-    const uint32_t nt = __ldg(A.n_tiles);
 
     if (warp == kCW) {
         // ---------------- producer warp: job -> bulk copies ----------------
+        const uint32_t nt = __ldg(A.n_tiles);
         const uint32_t* jw = reinterpret_cast<const uint32_t*>(p.jobs);
         uint32_t t = blockIdx.x;
-        uint32_t wcur = (t < nt && lane < 24) ? __ldg(jw + (size_t)t * 24 + lane) : 0u;
-        for (uint32_t it = 0; t < nt; ++it, t += gridDim.x) {
-            const uint32_t tn = t + gridDim.x;
-            const uint32_t wnext = (tn < nt && lane < 24) ? __ldg(jw + (size_t)tn * 24 + lane) : 0u;
+        bool have = t < nt;
+        uint32_t wcur = have ? __ldg(jw + (size_t)t * 32 + lane) : 0u;
+        uint32_t it = 0;
+        for (; have; ++it) {
+            // the next job: the chained one, else the first job of this CTA's next tile
+            const uint32_t next = __shfl_sync(kFull, wcur, 3);
+            uint32_t nidx = next;
+            bool nhave = true;
+            if (next == 0) { t += gridDim.x; nidx = t; nhave = t < nt; }
+            const uint32_t wnext = nhave ? __ldg(jw + (size_t)nidx * 32 + lane) : 0u;
+
             const int s = (int)(it % kStages);
             const unsigned ph = (it / kStages) & 1u;
             Stage& st = sm.st[s];
             const uint32_t a_first = __shfl_sync(kFull, wcur, 0), a_count = __shfl_sync(kFull, wcur, 1);
-            const uint32_t z_lo = __shfl_sync(kFull, wcur, 2), flags = __shfl_sync(kFull, wcur, 3);
-            const int nseg = (int)(flags & 0xFFu);
-            const int sb = 4 + 5 * min(lane, kSegs - 1);
-            const uint32_t row_lo = __shfl_sync(kFull, wcur, sb), cs_lo = __shfl_sync(kFull, wcur, sb + 1);
-            const uint32_t k_lo = __shfl_sync(kFull, wcur, sb + 2), n_ra = __shfl_sync(kFull, wcur, sb + 3);
-            const uint32_t nkr = __shfl_sync(kFull, wcur, sb + 4);
-            const uint32_t nk = nkr & 0xFFFFu, nr = nkr >> 16;
-            const bool segact = lane < nseg && nr != 0;
+            const uint32_t flags = __shfl_sync(kFull, wcur, 2);
+            const int nseg = (int)(flags & 0xFu);
+            const int sb = 4 + 8 * min(lane, kSegs - 1);
+            const uint32_t zone = __shfl_sync(kFull, wcur, sb), k_lo = __shfl_sync(kFull, wcur, sb + 1);
+            const uint32_t nk = __shfl_sync(kFull, wcur, sb + 2), row_lo = __shfl_sync(kFull, wcur, sb + 3);
+            const uint32_t nr = __shfl_sync(kFull, wcur, sb + 4), n_ra = __shfl_sync(kFull, wcur, sb + 5);
+            const uint32_t cs_lo = __shfl_sync(kFull, wcur, sb + 6), ctr = __shfl_sync(kFull, wcur, sb + 7);
+            const bool segact = lane < nseg;
             const uint32_t row_al = row_lo & ~1u, cs_al = cs_lo & ~3u;
             const uint32_t n_ld = segact ? (((row_lo + nr + 1u) & ~1u) - row_al) : 0u;
             const uint32_t c_ld = segact ? (((cs_lo + nk + 1u + 3u) & ~3u) - cs_al) : 0u;
@@ -388,15 +489,14 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
             const uint32_t a_ld = any ? (((a_first + a_count + 1u) & ~1u) - a_al) : 0u;
             const uint32_t bytes = a_ld * 40u + rtot * 32u + ctot * 4u;
 
-            mbar_wait(&sm.empty[s], ph ^ 1u);
-            if (lane == 0) {
-                st.d.a_first = a_first; st.d.a_count = a_count; st.d.a_off = a_first - a_al; st.d.flags = flags;
-                st.d.nseg = nseg; st.d.z_lo = (int32_t)z_lo;
-            }
-            if (lane < kSegs) {
+            mbar_wait_backoff(&sm.empty[s], ph ^ 1u);
+            if (lane == 0) { st.d.a_count = a_count; st.d.a_off = a_first - a_al; st.d.flags = flags; st.d.nseg = nseg; }
+            if (segact) {
                 SegDesc& e = st.d.seg[lane];
-                e.n_d = (double)(int32_t)n_ra; e.k_lo = (int32_t)k_lo; e.k_hi = (int32_t)(k_lo + nk) - 1;
-                e.cdelta = (int32_t)((cs_lo - k_lo) - cs_al + coff); e.rdelta = roff - row_al; e.n_rows = segact ? nr : 0u;
+                e.n_d = (double)(int32_t)n_ra; e.centre = (double)__uint_as_float(ctr);
+                e.zone = (int32_t)zone; e.k_lo = (int32_t)k_lo; e.k_hi = (int32_t)(k_lo + nk) - 1;
+                e.cdelta = (int32_t)((cs_lo - k_lo) - cs_al + coff); e.rdelta = roff - row_al;
+                e.row_lo = row_lo; e.row_hi = row_lo + nr;
             }
             __syncwarp();
             if (lane == 0) { if (bytes) mbar_arrive_expect_tx(&sm.full[s], bytes); else mbar_arrive(&sm.full[s]); }
@@ -414,8 +514,12 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
                 void* dst = k == 0 ? (void*)st.ax : k == 1 ? (void*)st.ay : k == 2 ? (void*)st.az : k == 3 ? (void*)st.apos : (void*)st.aid;
                 bulk_g2s(dst, src, a_ld * 8u, &sm.full[s]);
             }
-            wcur = wnext;
+            wcur = wnext; have = nhave;
         }
+        // tell the consumers that nothing follows
+        const int s = (int)(it % kStages);
+        mbar_wait_backoff(&sm.empty[s], ((it / kStages) & 1u) ^ 1u);
+        if (lane == 0) { sm.st[s].d.flags = kJobEnd; sm.st[s].d.nseg = 0; sm.st[s].d.a_count = 0; mbar_arrive(&sm.full[s]); }
         return;
     }
 
@@ -423,52 +527,73 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
     const GridView& g = B.g;
     WarpQueue& q = sm.q[warp];
     unsigned qn = 0;
-    uint32_t it = 0;
-    for (uint32_t t = blockIdx.x; t < nt; t += gridDim.x, ++it) {
+    Best best; best.has = false; best.c2 = 0.0; best.idb = 0;
+    for (uint32_t it = 0;; ++it) {
         const int s = (int)(it % kStages);
         const unsigned ph = (it / kStages) & 1u;
         mbar_wait(&sm.full[s], ph);
         const Stage& st = sm.st[s];
         const StageDesc& d = st.d;
         const uint32_t flags = d.flags, a_count = d.a_count;
+        if (flags & kJobEnd) break;
         const int nseg = d.nseg;
-        if ((nseg != 0 || (flags & kJobDirect)) && (uint32_t)(warp * 32) < a_count) {
+        if ((uint32_t)(warp * 32) < a_count) {
             const bool act = threadIdx.x < a_count;
-            const unsigned ra = act ? threadIdx.x + d.a_off : d.a_off;
-            const double ax = st.ax[ra], ay = st.ay[ra], az = st.az[ra];
-            const float2 pf = st.apos[ra];
-            const long long ida = st.aid[ra];
-            Best best; best.has = false; best.c2 = 0.0; best.idb = 0;
-            if (flags & kJobDirect) {
-                if (act) scan_general<MODE>(B, p, ida, ax, ay, az, pf, best);
-                __syncwarp();
-            } else {
-                const double dlo = (double)pf.y - p.pad_dec, dhi = (double)pf.y + p.pad_dec;
-                const int zlo = zone_of(g, dlo) - d.z_lo, zhi = zone_of(g, dhi) - d.z_lo;
-                const float fx = (float)ax, fy = (float)ay;
-                const float sn = p.sin_r_up * rsqrtf(fx * fx + fy * fy);
-                const double w = (double)(sn * (1.011f * 57.29577951f)) + kEpsRaDeg;
-                const double u = box_u(g, (double)pf.x);
-                const double vlo = (u - w) * g.inv_span, vhi = (u + w) * g.inv_span;
-                unsigned p0 = 0, p1 = 0, s0 = 0, s1 = 0;      // a lane's first and (zone-spanning rows) second range
-                for (int sg = 0; sg < nseg; ++sg) {
-                    const SegDesc& e = d.seg[sg];
-                    if (e.n_rows == 0) continue;
-                    int k0 = __double2int_rd(vlo * e.n_d), k1 = __double2int_rd(vhi * e.n_d);
-                    k0 = min(max(k0, e.k_lo), e.k_hi); k1 = min(max(k1, e.k_lo), e.k_hi);
-                    const unsigned q0 = st.cs[k0 + e.cdelta] + e.rdelta, q1 = st.cs[k1 + 1 + e.cdelta] + e.rdelta;
-                    const bool has = act && sg >= zlo && sg <= zhi && q1 > q0;
-                    if (sg >= 2 && __any_sync(kFull, has && p1 > p0 && s1 > s0)) {      // a third range: drain first
-                        scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, p0, p1, best, lane);
-                        scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, s0, s1, best, lane);
-                        p0 = p1 = s0 = s1 = 0;
+            if (MODE == HLC2_NEAREST && (flags & kJobFirst)) best.has = false;
+            long long ida = 0;
+            if (nseg != 0 || (flags & kJobDirect)) {
+                const unsigned ra = act ? threadIdx.x + d.a_off : d.a_off;
+                const double ax = st.ax[ra], ay = st.ay[ra], az = st.az[ra];
+                const float2 pf = st.apos[ra];
+                ida = st.aid[ra];
+                if (flags & kJobDirect) {
+                    if (act) scan_general<MODE>(B, p, ida, ax, ay, az, pf, best);
+                    __syncwarp();
+                } else {
+                    const double dlo = (double)pf.y - p.pad_dec, dhi = (double)pf.y + p.pad_dec;
+                    const int zlo = zone_of(g, dlo), zhi = zone_of(g, dhi);
+                    const float fx = (float)ax, fy = (float)ay;
+                    const float sn = p.sin_r_up * rsqrtf(fx * fx + fy * fy);
+                    const double w = (double)(sn * (1.011f * 57.29577951f)) + kEpsRaDeg;
+                    const double u = box_u(g, (double)pf.x);
+                    const double vlo0 = (u - w) * g.inv_span, vhi0 = (u + w) * g.inv_span;
+                    unsigned p0 = 0, p1 = 0, s0 = 0, s1 = 0;      // a lane's first and (zone-spanning rows) second range
+                    for (int sg = 0; sg < nseg; ++sg) {
+                        const SegDesc& e = d.seg[sg];
+                        bool has = act && e.zone >= zlo && e.zone <= zhi;
+                        int k0, k1;
+                        if (flags & kJobRing) { k0 = e.k_lo; k1 = e.k_hi; }
+                        else {
+                            double vlo = vlo0, vhi = vhi0;
+                            if (flags & kJobWrap) {           // re-centre this row's RA on the piece, then clip to the box
+                                double dd = u - e.centre;
+                                dd = dd > 180.0 ? dd - 360.0 : (dd < -180.0 ? dd + 360.0 : dd);
+                                const double lo = e.centre + dd - w, hi = e.centre + dd + w;
+                                has = has && hi >= 0.0 && lo <= g.span;
+                                vlo = fmax(lo, 0.0) * g.inv_span; vhi = fmin(hi, g.span) * g.inv_span;
+                            }
+                            k0 = __double2int_rd(vlo * e.n_d); k1 = __double2int_rd(vhi * e.n_d);
+                            has = has && k1 >= e.k_lo && k0 <= e.k_hi;
+                            k0 = min(max(k0, e.k_lo), e.k_hi); k1 = min(max(k1, e.k_lo), e.k_hi);
+                        }
+                        unsigned q0 = st.cs[k0 + e.cdelta], q1 = st.cs[k1 + 1 + e.cdelta];
+                        q0 = min(max(q0, e.row_lo), e.row_hi) + e.rdelta; q1 = min(max(q1, e.row_lo), e.row_hi) + e.rdelta;
+                        has = has && q1 > q0;
+                        if (sg >= 2 && __any_sync(kFull, has && p1 > p0 && s1 > s0)) {      // a third range: drain first
+                            scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, p0, p1, best, lane);
+                            scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, s0, s1, best, lane);
+                            p0 = p1 = s0 = s1 = 0;
+                        }
+                        if (has) { if (p1 == p0) { p0 = q0; p1 = q1; } else { s0 = q0; s1 = q1; } }
                     }
-                    if (has) { if (p1 == p0) { p0 = q0; p1 = q1; } else { s0 = q0; s1 = q1; } }
+                    scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, p0, p1, best, lane);
+                    if (__any_sync(kFull, s1 > s0)) scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, s0, s1, best, lane);
                 }
-                scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, p0, p1, best, lane);
-                if (__any_sync(kFull, s1 > s0)) scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, s0, s1, best, lane);
             }
-            if (MODE == HLC2_NEAREST) push_hits(p, q, qn, best.has, ida, best.idb, best.c2, lane);
+            if (MODE == HLC2_NEAREST && (flags & kJobLast)) {
+                if (nseg == 0 && !(flags & kJobDirect)) ida = st.aid[act ? threadIdx.x + d.a_off : d.a_off];
+                push_hits(p, q, qn, act && best.has, ida, best.idb, best.c2, lane);
+            }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm.empty[s]);
@@ -477,7 +602,11 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
     if (qn) flush_rows(p, q, 0, qn, lane);
 }
 
-size_t match_temp_bytes(const IndexView& A, const IndexView&) { return ((size_t)A.tile_cap + 1) * sizeof(Job); }
+static inline size_t pool_cap_of(size_t tile_cap) { return 3 * tile_cap + 4096; }
+
+size_t match_temp_bytes(const IndexView& A, const IndexView&) {
+    return ((size_t)A.tile_cap + pool_cap_of(A.tile_cap)) * sizeof(Job) + 256;
+}
 
 void launch_match(const IndexView& A, const IndexView& B, double radius_arcsec, int mode,
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
@@ -491,8 +620,11 @@ void launch_match(const IndexView& A, const IndexView& B, double radius_arcsec, 
     p.pad_dec = p.r_deg + kEpsDecDeg;
     p.sin_r_up = (float)((double)sinl(r_rad) * (1.0 + 1e-5));
     p.out_ida = out_ida; p.out_idb = out_idb; p.out_sep = out_sep; p.capacity = capacity; p.count = d_count;
-    Job* jobs = reinterpret_cast<Job*>(d_temp);
-    p.jobs = jobs;
+    const size_t tiles = A.tile_cap;
+    p.jobs = reinterpret_cast<Job*>(d_temp);
+    p.tile_cap = (uint32_t)tiles; p.pool_cap = (uint32_t)pool_cap_of(tiles);
+    p.pool_count = reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(d_temp) + (tiles + pool_cap_of(tiles)) * sizeof(Job));
+    cudaMemsetAsync(p.pool_count, 0, sizeof(uint32_t), s);
     const int m = mode == HLC2_NEAREST ? 1 : 0;
     static int per_sm[2] = {0, 0};
     const size_t smem = sizeof(MatchSmem);
@@ -507,9 +639,8 @@ void launch_match(const IndexView& A, const IndexView& B, double radius_arcsec, 
         }
         per_sm[m] = v > 0 ? v : 1;
     }
-    const size_t tiles = A.tile_cap;
     const unsigned pblocks = (unsigned)std::min<size_t>((tiles + 127) / 128, (size_t)sm_count() * 8);
-    k_plan<<<pblocks, 128, 0, s>>>(A, B, p, jobs);
+    k_plan<<<pblocks, 128, 0, s>>>(A, B, p);
     count_launch();
     // persistent grid: SM count x resident CTAs, never more CTAs than tiles
     const unsigned blocks = (unsigned)std::max<size_t>(1, std::min<size_t>(tiles, (size_t)sm_count() * per_sm[m]));
