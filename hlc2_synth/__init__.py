@@ -330,3 +330,15 @@ def stress_classes(k_seed: int, n: int, grid: dict | None = None):
     for j, m in _chunks(n):
         out.append(stress_mix(_rng(k_seed, 0, j), m, g)[2])
     return np.concatenate(out)
+
+
+def to_bands(cat: "Catalogue", band_edges_deg: np.ndarray):
+    """Bucket a catalogue into declination bands (input preparation for the streaming entry point: band k holds
+    dec in [edges[k], edges[k+1]), the last band closed above).  Returns (Catalogue in band order, int64 offsets)."""
+    edges = np.asarray(band_edges_deg, np.float64)
+    nb = len(edges) - 1
+    k = np.clip(np.searchsorted(edges, cat.dec, side="right") - 1, 0, nb - 1)
+    order = np.argsort(k, kind="stable")
+    off = np.zeros(nb + 1, np.int64)
+    np.cumsum(np.bincount(k, minlength=nb), out=off[1:])
+    return cat.take(order), off

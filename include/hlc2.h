@@ -172,7 +172,14 @@ int hlc2_crossmatch(const hlc2_index* A, const hlc2_index* B, double radius_arcs
  *                  h_a_id / h_b_id may be NULL (ids = global row numbers).
  *   d_arena        caller's device scratch of arena_bytes (see hlc2_stream_sizes).
  *   h_out_*        pinned outputs of `capacity` rows; *h_count receives the total found.
- * Synchronous: returns when the outputs are complete.
+ *   max_band_out   rows of one band's result the device output slots hold (as given to hlc2_stream_sizes).
+ * The B window of band k is band k plus the rows of bands k-1 / k+1 within radius of band k's edges
+ * (selected on the device), so every A source sees one window and nearest mode needs no merge.
+ * ids NULL: ids are the global row numbers of the banded arrays.
+ * Synchronous: returns when the outputs are complete.  HLC2_ERR_BUFFER_TOO_SMALL if a band found more than
+ * max_band_out rows or the total exceeded capacity (*h_count still holds the full count: retry larger);
+ * HLC2_ERR_BAD_COORD if a band held an invalid coordinate (the other rows are matched as usual);
+ * HLC2_ERR_INVALID_ARG for a band lower than the radius (n_bands > 1), unordered edges or offsets.
  */
 int hlc2_stream_sizes(int64_t max_band_a, int64_t max_band_b, const hlc2_opts* opts, int64_t max_band_out,
                       size_t* arena_bytes);

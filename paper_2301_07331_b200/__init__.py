@@ -245,6 +245,40 @@ def crossmatch(A: Index, B: Index, radius_arcsec: float, mode: int = HLC2_ALL_PA
     raise RuntimeError("crossmatch: result count changed between runs")
 
 
+
+def hlc2_stream_sizes(max_band_a: int, max_band_b: int, opts: hlc2_opts | None, max_band_out: int) -> int:
+    ab = ctypes.c_size_t(0)
+    rc = lib().hlc2_stream_sizes(int(max_band_a), int(max_band_b), ctypes.byref(opts) if opts is not None else None,
+                                 int(max_band_out), ctypes.byref(ab))
+    if rc != HLC2_OK:
+        raise Hlc2Error(rc, "hlc2_stream_sizes")
+    return ab.value
+
+
+def hlc2_stream_crossmatch(a_cols, a_off, b_cols, b_off, band_edges_deg, radius_arcsec: float, mode: int,
+                           opts: hlc2_opts, out_ida, out_idb, out_sep, arena, max_band_out: int) -> int:
+    """Raw call.  a_cols / b_cols = (ra, dec, id-or-None) PINNED host tensors already bucketed into declination
+    bands; a_off / b_off / band_edges_deg host tensors (int64 / int64 / float64, n_bands + 1 entries); out_* pinned
+    host tensors; arena a CUDA uint8 tensor of hlc2_stream_sizes bytes.  Synchronous.  Returns the rows found
+    (the first min(found, capacity) of them are in out_*); raises if a buffer was too small."""
+    torch = _torch()
+    for t in (*a_cols, *b_cols, out_ida, out_idb, out_sep):
+        assert t is None or (t.device.type == "cpu" and t.is_pinned() and t.is_contiguous()), "pinned host tensors expected"
+    n_bands = int(band_edges_deg.numel()) - 1
+    assert a_off.numel() == n_bands + 1 and b_off.numel() == n_bands + 1
+    ptr = lambda t: t.data_ptr() if t is not None else None
+    cnt = ctypes.c_ulonglong(0)
+    rc = lib().hlc2_stream_crossmatch(ptr(a_cols[0]), ptr(a_cols[1]), ptr(a_cols[2]), a_off.data_ptr(),
+                                      ptr(b_cols[0]), ptr(b_cols[1]), ptr(b_cols[2]), b_off.data_ptr(),
+                                      band_edges_deg.data_ptr(), n_bands, float(radius_arcsec), int(mode),
+                                      ctypes.byref(opts), out_ida.data_ptr(), out_idb.data_ptr(), out_sep.data_ptr(),
+                                      int(out_ida.shape[0]), ctypes.byref(cnt), arena.data_ptr(), arena.numel(),
+                                      int(max_band_out))
+    if rc != HLC2_OK:
+        e = Hlc2Error(rc, "hlc2_stream_crossmatch"); e.found = cnt.value
+        raise e
+    return int(cnt.value)
+
 def kernel_launches() -> int:
     return int(lib().hlc2_kernel_launches())
 

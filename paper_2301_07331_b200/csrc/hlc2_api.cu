@@ -130,6 +130,15 @@ static TempLayout make_temp(int64_t n, const Layout& L) {
     return T;
 }
 
+namespace hlc2 {
+size_t match_temp_bound(int64_t n_a, const hlc2_opts* opts) {
+    hlc2_opts o = opts_or_default(opts);
+    o.grid_like = nullptr;
+    Layout L = make_layout(n_a, o);
+    return match_temp_for_tiles(L.cap_tiles);
+}
+}  // namespace hlc2
+
 // ---- the planner: grid from the catalogue's extent and density (host, O(n_zones)) ----------
 static void fill_zones(HostGrid& g, double c_arcsec) {
     const double c_rad = c_arcsec / 206264.80624709636;

@@ -82,6 +82,9 @@ void launch_tiles(const uint32_t* cell_start, const uint32_t* cell_base, uint32_
                   uint32_t tile_cap, uint32_t* d_tile_first, TileDesc* tiles, uint32_t* d_n_tiles, cudaStream_t s);
 
 size_t match_temp_bytes(const IndexView& A, const IndexView& B);
+size_t match_temp_for_tiles(size_t tile_cap);
+// upper bound of hlc2_crossmatch_sizes for any A index of <= n sources built with these options (hlc2_api.cu)
+size_t match_temp_bound(int64_t n_a, const hlc2_opts* opts);
 void launch_match(const IndexView& A, const IndexView& B, double radius_arcsec, int mode,
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
                   unsigned long long* d_count, void* d_temp, cudaStream_t s);

@@ -604,9 +604,8 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
 
 static inline size_t pool_cap_of(size_t tile_cap) { return 3 * tile_cap + 4096; }
 
-size_t match_temp_bytes(const IndexView& A, const IndexView&) {
-    return ((size_t)A.tile_cap + pool_cap_of(A.tile_cap)) * sizeof(Job) + 256;
-}
+size_t match_temp_for_tiles(size_t tile_cap) { return (tile_cap + pool_cap_of(tile_cap)) * sizeof(Job) + 256; }
+size_t match_temp_bytes(const IndexView& A, const IndexView&) { return match_temp_for_tiles(A.tile_cap); }
 
 void launch_match(const IndexView& A, const IndexView& B, double radius_arcsec, int mode,
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
