@@ -15,7 +15,10 @@ constexpr uint32_t kMaxN = (1u << 30) - 1;    // the radix sort's chained scan k
 constexpr int kRadixBits = 9;                 // LSD radix sort digit
 constexpr int kRadix = 1 << kRadixBits;
 constexpr int kMaxPasses = 4;                 // 32-bit keys
-constexpr int kTile = 128;                    // sources per match tile (= threads of the match CTA)
+#ifndef HLC2_TILE
+#define HLC2_TILE 128
+#endif
+constexpr int kTile = HLC2_TILE;                    // sources per match tile (= threads of the match CTA)
 
 // ---- grid as the kernels see it (passed by value) ----------------------------------------
 struct GridView {

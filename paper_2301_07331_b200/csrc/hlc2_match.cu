@@ -28,6 +28,8 @@
 // Decisions are fp64; the fp32 estimate only ever selects a superset of cells.
 #include <math.h>
 
+#include <algorithm>
+
 #include "hlc2_grid.cuh"
 
 namespace hlc2 {
@@ -125,25 +127,17 @@ __device__ __forceinline__ void mbar_arrive(unsigned long long* b) {
 __device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* b, unsigned bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
 }
+// try_wait suspends the thread in hardware until the phase completes or the time hint (ns) runs out, so a long
+// hint costs no wake-up latency and spares the issue slots a polling loop would burn
 __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) {
     const uint32_t a = smem_u32(b);
     unsigned done;
     do {
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(done) : "r"(a), "r"(parity) : "memory");
+        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n selp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(done) : "r"(a), "r"(parity), "r"(0x4000u) : "memory");
     } while (!done);
 }
-// the producer runs ahead and mostly waits for a free stage: back off between polls so that it does not eat issue slots
-__device__ __forceinline__ void mbar_wait_backoff(unsigned long long* b, unsigned parity) {
-    const uint32_t a = smem_u32(b);
-    unsigned done;
-    for (;;) {
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(done) : "r"(a), "r"(parity) : "memory");
-        if (done) break;
-        __nanosleep(256);
-    }
-}
+__device__ __forceinline__ void mbar_wait_backoff(unsigned long long* b, unsigned parity) { mbar_wait(b, parity); }
 // global -> shared bulk copy, completion counted in bytes on an mbarrier; 16-byte aligned src, dst and size
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* b) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -430,6 +424,43 @@ __device__ __forceinline__ void scan_staged(const Stage& st, const MatchArgs& p,
     }
 }
 
+// a lane's row ranges in the pieces of a job.  GENERAL: ring and wrap jobs (polar tiles, windows through u = 0 / 360).
+template <int MODE, bool GENERAL>
+__device__ __forceinline__ void seg_ranges(const Stage& st, const MatchArgs& p, WarpQueue& q, unsigned& qn, const GridView& g,
+                                           uint32_t flags, int nseg, bool act, int zlo, int zhi, double u, double w,
+                                           double vlo0, double vhi0, long long ida, double ax, double ay, double az,
+                                           Best& best, int lane, unsigned& p0, unsigned& p1, unsigned& s0, unsigned& s1) {
+    const StageDesc& d = st.d;
+    for (int sg = 0; sg < nseg; ++sg) {
+        const SegDesc& e = d.seg[sg];
+        bool has = act && e.zone >= zlo && e.zone <= zhi;
+        int k0, k1;
+        if (GENERAL && (flags & kJobRing)) { k0 = e.k_lo; k1 = e.k_hi; }
+        else {
+            double vlo = vlo0, vhi = vhi0;
+            if (GENERAL && (flags & kJobWrap)) {           // re-centre this row's RA on the piece, then clip to the box
+                double dd = u - e.centre;
+                dd = dd > 180.0 ? dd - 360.0 : (dd < -180.0 ? dd + 360.0 : dd);
+                const double lo = e.centre + dd - w, hi = e.centre + dd + w;
+                has = has && hi >= 0.0 && lo <= g.span;
+                vlo = fmax(lo, 0.0) * g.inv_span; vhi = fmin(hi, g.span) * g.inv_span;
+            }
+            k0 = __double2int_rd(vlo * e.n_d); k1 = __double2int_rd(vhi * e.n_d);
+            has = has && k1 >= e.k_lo && k0 <= e.k_hi;
+            k0 = min(max(k0, e.k_lo), e.k_hi); k1 = min(max(k1, e.k_lo), e.k_hi);
+        }
+        unsigned q0 = st.cs[k0 + e.cdelta], q1 = st.cs[k1 + 1 + e.cdelta];
+        q0 = min(max(q0, e.row_lo), e.row_hi) + e.rdelta; q1 = min(max(q1, e.row_lo), e.row_hi) + e.rdelta;
+        has = has && q1 > q0;
+        if (sg >= 2 && __any_sync(kFull, has && p1 > p0 && s1 > s0)) {      // a third range: drain first
+            scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, p0, p1, best, lane);
+            scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, s0, s1, best, lane);
+            p0 = p1 = s0 = s1 = 0;
+        }
+        if (has) { if (p1 == p0) { p0 = q0; p1 = q1; } else { s0 = q0; s1 = q1; } }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------------
 // k_match
 // ------------------------------------------------------------------------------------------------------
@@ -450,17 +481,25 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
         // ---------------- producer warp: job -> bulk copies ----------------
         const uint32_t nt = __ldg(A.n_tiles);
         const uint32_t* jw = reinterpret_cast<const uint32_t*>(p.jobs);
+        // first jobs of this CTA's tiles are fetched two tiles ahead (one word per lane), so the producer never waits
+        // on them; only a chained job (a tile whose window did not fit one stage) is fetched on demand
         uint32_t t = blockIdx.x;
+        const uint32_t G = gridDim.x;
         bool have = t < nt;
         uint32_t wcur = have ? __ldg(jw + (size_t)t * 32 + lane) : 0u;
+        uint32_t w1 = (t + G < nt) ? __ldg(jw + (size_t)(t + G) * 32 + lane) : 0u;
+        uint32_t w2 = (t + 2 * G < nt) ? __ldg(jw + (size_t)(t + 2 * G) * 32 + lane) : 0u;
         uint32_t it = 0;
         for (; have; ++it) {
-            // the next job: the chained one, else the first job of this CTA's next tile
             const uint32_t next = __shfl_sync(kFull, wcur, 3);
-            uint32_t nidx = next;
+            uint32_t wnext;
             bool nhave = true;
-            if (next == 0) { t += gridDim.x; nidx = t; nhave = t < nt; }
-            const uint32_t wnext = nhave ? __ldg(jw + (size_t)nidx * 32 + lane) : 0u;
+            if (next != 0) wnext = __ldg(jw + (size_t)next * 32 + lane);
+            else {
+                t += G; nhave = t < nt;
+                wnext = w1; w1 = w2;
+                w2 = (t + 2 * G < nt) ? __ldg(jw + (size_t)(t + 2 * G) * 32 + lane) : 0u;
+            }
 
             const int s = (int)(it % kStages);
             const unsigned ph = (it / kStages) & 1u;
@@ -537,7 +576,11 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
         const uint32_t flags = d.flags, a_count = d.a_count;
         if (flags & kJobEnd) break;
         const int nseg = d.nseg;
+#ifdef HLC2_EXP_NOCOMPUTE
+        if (false) {
+#else
         if ((uint32_t)(warp * 32) < a_count) {
+#endif
             const bool act = threadIdx.x < a_count;
             if (MODE == HLC2_NEAREST && (flags & kJobFirst)) best.has = false;
             long long ida = 0;
@@ -558,34 +601,10 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
                     const double u = box_u(g, (double)pf.x);
                     const double vlo0 = (u - w) * g.inv_span, vhi0 = (u + w) * g.inv_span;
                     unsigned p0 = 0, p1 = 0, s0 = 0, s1 = 0;      // a lane's first and (zone-spanning rows) second range
-                    for (int sg = 0; sg < nseg; ++sg) {
-                        const SegDesc& e = d.seg[sg];
-                        bool has = act && e.zone >= zlo && e.zone <= zhi;
-                        int k0, k1;
-                        if (flags & kJobRing) { k0 = e.k_lo; k1 = e.k_hi; }
-                        else {
-                            double vlo = vlo0, vhi = vhi0;
-                            if (flags & kJobWrap) {           // re-centre this row's RA on the piece, then clip to the box
-                                double dd = u - e.centre;
-                                dd = dd > 180.0 ? dd - 360.0 : (dd < -180.0 ? dd + 360.0 : dd);
-                                const double lo = e.centre + dd - w, hi = e.centre + dd + w;
-                                has = has && hi >= 0.0 && lo <= g.span;
-                                vlo = fmax(lo, 0.0) * g.inv_span; vhi = fmin(hi, g.span) * g.inv_span;
-                            }
-                            k0 = __double2int_rd(vlo * e.n_d); k1 = __double2int_rd(vhi * e.n_d);
-                            has = has && k1 >= e.k_lo && k0 <= e.k_hi;
-                            k0 = min(max(k0, e.k_lo), e.k_hi); k1 = min(max(k1, e.k_lo), e.k_hi);
-                        }
-                        unsigned q0 = st.cs[k0 + e.cdelta], q1 = st.cs[k1 + 1 + e.cdelta];
-                        q0 = min(max(q0, e.row_lo), e.row_hi) + e.rdelta; q1 = min(max(q1, e.row_lo), e.row_hi) + e.rdelta;
-                        has = has && q1 > q0;
-                        if (sg >= 2 && __any_sync(kFull, has && p1 > p0 && s1 > s0)) {      // a third range: drain first
-                            scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, p0, p1, best, lane);
-                            scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, s0, s1, best, lane);
-                            p0 = p1 = s0 = s1 = 0;
-                        }
-                        if (has) { if (p1 == p0) { p0 = q0; p1 = q1; } else { s0 = q0; s1 = q1; } }
-                    }
+                    if (flags & (kJobRing | kJobWrap))
+                        seg_ranges<MODE, true>(st, p, q, qn, g, flags, nseg, act, zlo, zhi, u, w, vlo0, vhi0, ida, ax, ay, az, best, lane, p0, p1, s0, s1);
+                    else
+                        seg_ranges<MODE, false>(st, p, q, qn, g, flags, nseg, act, zlo, zhi, u, w, vlo0, vhi0, ida, ax, ay, az, best, lane, p0, p1, s0, s1);
                     scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, p0, p1, best, lane);
                     if (__any_sync(kFull, s1 > s0)) scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, s0, s1, best, lane);
                 }
@@ -605,12 +624,20 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
 static inline size_t pool_cap_of(size_t tile_cap) { return 3 * tile_cap + 4096; }
 
 size_t match_temp_for_tiles(size_t tile_cap) { return (tile_cap + pool_cap_of(tile_cap)) * sizeof(Job) + 256; }
-size_t match_temp_bytes(const IndexView& A, const IndexView&) { return match_temp_for_tiles(A.tile_cap); }
+size_t match_temp_bytes(const IndexView& A, const IndexView& B) { return match_temp_for_tiles(std::max(A.tile_cap, B.tile_cap)); }
 
-void launch_match(const IndexView& A, const IndexView& B, double radius_arcsec, int mode,
+void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_arcsec, int mode,
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
                   unsigned long long* d_count, void* d_temp, cudaStream_t s) {
-    if (A.n == 0 || B.n == 0) return;
+    if (A_in.n == 0 || B_in.n == 0) return;
+    // all_pairs is symmetric: the pair set of (A, B) is that of (B, A) with the id columns exchanged.  The per-row
+    // work (window, cell look-ups) is paid by the catalogue whose rows drive the lanes, while staging grows with the
+    // scanned rows per driving row; measured on config 3 (ratio 2) the two directions tie, so the roles are
+    // exchanged only when B is much the smaller catalogue.
+    const bool swap = mode == HLC2_ALL_PAIRS && (size_t)B_in.n * 3 < (size_t)A_in.n;
+    const IndexView& A = swap ? B_in : A_in;
+    const IndexView& B = swap ? A_in : B_in;
+    if (swap) std::swap(out_ida, out_idb);
     MatchArgs p;
     long double r_rad = (long double)radius_arcsec * (3.141592653589793238462643383279502884L / 648000.0L);
     long double hs = sinl(0.5L * r_rad);
