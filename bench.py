@@ -50,7 +50,7 @@ def peak_hbm():
 
 def ncu_traffic():
     """DRAM bytes per launch of the match kernel from the committed ncu --set full capture, or None."""
-    p = os.path.join(ROOT, "profiles", "match_traffic.json")
+    p = os.path.join(ROOT, "profiles", "match_traffic.txt")
     try:
         return json.load(open(p))
     except Exception:
