@@ -1,29 +1,30 @@
 // hlc2_match.cu -- the match kernels (NS (b)).
 //
-// Work unit = one A tile: up to kTile consecutive cell-sorted A rows of one A zone (the role of the paper's
-// calculation blocks).  Two kernels:
+// Work unit = one A tile: up to kTile consecutive cell-sorted A rows of one A zone.  Two kernels:
 //
 //   k_plan   one thread per A tile.  From the tile's own cell bounds (exact: zone edges and RA-cell edges of
 //            A's grid) it derives the window on B's grid that any row of the tile can reach:
-//              dec  [dec_lo - r, dec_hi + r]                          -> <= kSegs consecutive zones of B's grid
-//              RA   [ra_lo - W, ra_hi + W], W = asin(sin r / cos dec*) -> ONE contiguous cell range per zone
-//            (the cells the quad-direction strategy probes, L122-169, plus the diagonal neighbours and the
-//            1/cos(dec) widening it omits, so no pair is lost: the "No Index" result, L344) and writes a job:
-//            per zone the B row range and the slice of cell_start that covers it.  Tiles whose window wraps
-//            through RA = 0/360, touches a polar ring, needs more zones or more rows than a stage holds are
-//            marked DIRECT.
-//   k_match  persistent CTAs of kCW consumer warps + 1 producer warp, kStages-deep mbarrier ring.  The producer
-//            warp turns each job into 1-D bulk copies (cp.async.bulk, the TMA engine): the A tile (x, y, z,
-//            pos, id) and, per zone segment, B's x, y, z, id rows and the cell_start slice -- all contiguous
-//            because keys are zone-major / RA-minor.  Consumers: one lane per A row (the paper's
-//            thread-per-A-record hierarchy, L271-276).  A lane locates its own cells from the fp32 (ra, dec)
-//            estimate padded by a rigorous error bound, clips them to the job's range (the job covers every
-//            cell a row of the tile needs, so clipping never loses one), reads its row range from the staged
-//            cell_start slice and tests the staged rows: chord^2 <= 4 sin^2(r/2), all fp64 from shared memory.
-//            Hits (the role of d_out_dis, L282) are compacted by ballot + popcount into a per-warp queue of
-//            (idA, idB, chord^2) and flushed 64 at a time: one global atomic, coalesced stores, sep computed
-//            on full warps.  DIRECT tiles run the general per-lane path from global memory (any number of
-//            zones, RA wrap, polar rings).
+//              dec  [dec_lo - r, dec_hi + r]                           -> consecutive zones of B's grid
+//              RA   [ra_lo - W, ra_hi + W], W >= asin(sin r / cos dec*) -> one cell range per zone, a second one
+//                   when the window passes RA = 0/360, the whole ring at the poles
+//            (the cells the quad-direction strategy probes, plus the diagonal neighbours and
+//            the 1/cos(dec) widening it omits, so no pair is lost: the "No Index" result, L344).  The window is
+//            cut into pieces (zone, cell range, B row range) and the pieces are packed into jobs that fit one
+//            shared-memory stage -- the role of the paper's calculation blocks, L253-257, which were cut to fit
+//            device memory.  jobs[t] is the first job of tile t; further jobs hang off it through `next`.
+//            Only a tile that reaches more than kMaxZones zones of B's grid (B far denser than A) or that finds
+//            the job pool full is marked DIRECT.
+//   k_match  persistent CTAs of kCW consumer warps + 1 producer warp around a kStages-deep mbarrier ring.  The
+//            producer warp turns each job into 1-D bulk copies (cp.async.bulk, the TMA engine): the A tile (x, y,
+//            z, pos, id) and, per piece, B's x, y, z, id rows and the cell_start slice -- all contiguous because
+//            keys are zone-major / RA-minor.  Consumers: one lane per A row (the paper's thread-per-A-record
+//            hierarchy, L271-276).  A lane locates its own cells from the fp32 (ra, dec) estimate padded by a
+//            rigorous error bound, clips them to the piece (the jobs of a tile cover every cell a row of the tile
+//            needs, so clipping never loses one), reads its row range from the staged cell_start slice and tests
+//            the staged rows: chord^2 <= 4 sin^2(r/2), all fp64 from shared memory, two candidates per step
+//            without branches.  Hits (the role of d_out_dis, L282) are compacted by ballot + popcount into a
+//            per-warp queue of (idA, idB, chord^2) and flushed 32 at a time: one global atomic, coalesced stores,
+//            sep computed on full warps.  DIRECT tiles run the general per-lane path from global memory.
 //
 // Decisions are fp64; the fp32 estimate only ever selects a superset of cells.
 #include <math.h>
