@@ -648,9 +648,10 @@ void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_ar
     p.sin_r_up = (float)((double)sinl(r_rad) * (1.0 + 1e-5));
     p.out_ida = out_ida; p.out_idb = out_idb; p.out_sep = out_sep; p.capacity = capacity; p.count = d_count;
     const size_t tiles = A.tile_cap;
-    p.jobs = reinterpret_cast<Job*>(d_temp);
+    // scratch: 256-byte header (pool counter), then the tiles' first jobs, then the pool of chained jobs
+    p.pool_count = reinterpret_cast<uint32_t*>(d_temp);
+    p.jobs = reinterpret_cast<Job*>(reinterpret_cast<char*>(d_temp) + 256);
     p.tile_cap = (uint32_t)tiles; p.pool_cap = (uint32_t)pool_cap_of(tiles);
-    p.pool_count = reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(d_temp) + (tiles + pool_cap_of(tiles)) * sizeof(Job));
     cudaMemsetAsync(p.pool_count, 0, sizeof(uint32_t), s);
     const int m = mode == HLC2_NEAREST ? 1 : 0;
     static int per_sm[2] = {0, 0};

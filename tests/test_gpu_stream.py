@@ -102,3 +102,14 @@ def test_stream_argument_checks(P):
     assert cnt.value == 0
     assert L.hlc2_stream_crossmatch(*([None] * 9), 2, 1.0, 0, None, None, None, None, 0, ctypes.byref(cnt), None, 0, 0) == P.HLC2_ERR_INVALID_ARG
     assert L.hlc2_stream_crossmatch(*([None] * 9), 0, -1.0, 0, None, None, None, None, 0, ctypes.byref(cnt), None, 0, 0) == P.HLC2_ERR_INVALID_ARG
+
+
+def test_cfg5_streamed_nearest_scaled(P):
+    """Config 5 (streamed large, nearest) at a scale the oracle finishes in seconds: 2e5 x 1e5, 1-degree .. 30-degree bands."""
+    w = S.config(5, scale=1e-4)
+    assert w.modes == ("nearest",)
+    edges = np.array([-90.0, -45.0, -30.0, -29.0, -10.0, 0.0, 10.0, 30.0, 60.0, 90.0])
+    ga, gb, gs, *_ = stream_match(P, w.A, w.B, edges, w.radius_arcsec, 1)
+    oa, ob, os_, _ = oracle.match(w.A.ra, w.A.dec, w.A.id, w.B.ra, w.B.dec, w.B.id, w.radius_arcsec, 1)
+    rep = parity.compare_nearest((ga, gb, gs), (oa, ob, os_), w.radius_arcsec, parity.make_sep_of(w.A, w.B))
+    assert rep["n_gpu"] > 50_000
