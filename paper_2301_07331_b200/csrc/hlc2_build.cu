@@ -175,8 +175,11 @@ k_digit_scan(const uint32_t* __restrict__ digit_hist, uint32_t* __restrict__ dig
 }
 
 constexpr int kOsThreads = 512;                 // == kRadix: thread d owns digit d in the tile-level scans
-constexpr int kOsItems = 12;                    // even
-constexpr int kOsTile = kOsThreads * kOsItems;  // 6144 keys per tile
+#ifndef HLC2_OS_ITEMS
+#define HLC2_OS_ITEMS 18
+#endif
+constexpr int kOsItems = HLC2_OS_ITEMS;         // even
+constexpr int kOsTile = kOsThreads * kOsItems;  // 9216 keys per tile
 constexpr int kOsWarps = kOsThreads / 32;
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagIncl = 2u << 30, kFlagMask = 3u << 30;
 constexpr size_t kOsSmem = (size_t)(kOsWarps * kRadix + 2 * kOsTile) * 4;
