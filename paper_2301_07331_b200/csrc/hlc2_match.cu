@@ -16,15 +16,16 @@
 //            the job pool full is marked DIRECT.
 //   k_match  persistent CTAs of kCW consumer warps + 1 producer warp around a kStages-deep mbarrier ring.  The
 //            producer warp turns each job into 1-D bulk copies (cp.async.bulk, the TMA engine): the A tile (x, y,
-//            z, pos, id) and, per piece, B's x, y, z, id rows and the cell_start slice -- all contiguous because
+//            z, pos) and, per piece, B's x, y, z rows and the cell_start slice -- all contiguous because
 //            keys are zone-major / RA-minor.  Consumers: one lane per A row (the paper's thread-per-A-record
 //            hierarchy, L271-276).  A lane locates its own cells from the fp32 (ra, dec) estimate padded by a
 //            rigorous error bound, clips them to the piece (the jobs of a tile cover every cell a row of the tile
 //            needs, so clipping never loses one), reads its row range from the staged cell_start slice and tests
 //            the staged rows: chord^2 <= 4 sin^2(r/2), all fp64 from shared memory, two candidates per step
 //            without branches.  Hits (the role of d_out_dis, L282) are compacted by ballot + popcount into a
-//            per-warp queue of (idA, idB, chord^2) and flushed 32 at a time: one global atomic, coalesced stores,
-//            sep computed on full warps.  DIRECT tiles run the general per-lane path from global memory.
+//            per-warp queue of (A row, B row, chord^2) and flushed 32 at a time: one global atomic, the id
+//            look-ups, coalesced stores, sep computed on full warps.  DIRECT tiles run the general per-lane path
+//            from global memory.
 //
 // Decisions are fp64; the fp32 estimate only ever selects a superset of cells.
 #include <math.h>
@@ -50,7 +51,7 @@ constexpr int kMatchThreads = kTile + 32;    // + the producer warp
 #define HLC2_QCAP 64
 #endif
 #ifndef HLC2_CTAS
-#define HLC2_CTAS 5
+#define HLC2_CTAS 6
 #endif
 constexpr int kStages = HLC2_STAGES;
 constexpr int kSegs = 3;                     // window pieces per job
@@ -97,18 +98,18 @@ struct MatchArgs {
 };
 
 struct SegDesc { double n_d; double centre; int32_t zone, k_lo, k_hi, cdelta; uint32_t rdelta, row_lo, row_hi, pad; };
-struct StageDesc { uint32_t a_count, a_off, flags; int32_t nseg; SegDesc seg[kSegs]; };
+struct StageDesc { uint32_t a_first, a_count, a_off, flags; int32_t nseg; uint32_t pad; SegDesc seg[kSegs]; };
 
 struct __align__(16) Stage {
     double ax[kAPad], ay[kAPad], az[kAPad];
     float2 apos[kAPad];
-    long long aid[kAPad];
     double bx[kBCap + 2], by[kBCap + 2], bz[kBCap + 2];     // slot kBCap: a point no chord test can reach
-    long long bid[kBCap];
     uint32_t cs[kCsCap];
     StageDesc d;
 };
-struct WarpQueue { long long ida[kQCap], idb[kQCap]; double c2[kQCap]; };
+// ids are looked up when a queue is flushed (32 rows at a time, overlapped with the atomic), so neither catalogue's
+// id column is staged: the queue holds the global A and B row numbers
+struct WarpQueue { uint32_t a[kQCap], b[kQCap]; double c2[kQCap]; };
 struct __align__(16) MatchSmem {
     Stage st[kStages];
     WarpQueue q[kCW];
@@ -295,35 +296,34 @@ k_plan(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B,
 // the general per-lane path (DIRECT tiles): any number of zones, RA wrap, polar ring, window partly outside
 // B's box.  Reads B through global memory / L2.
 // ------------------------------------------------------------------------------------------------------
-struct Best { double c2; long long idb; bool has; };
+struct Best { double c2; uint32_t row; bool has; };      // row: global B row
 
 // one row straight to the output; lanes that arrive together share one global atomic
-__device__ __forceinline__ void emit_direct(const MatchArgs& p, long long ida, long long idb, double c2) {
+__device__ __forceinline__ void emit_direct(const IndexView& A, const IndexView& B, const MatchArgs& p, uint32_t a_row, uint32_t b_row, double c2) {
     const unsigned m = __activemask();
     const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
     unsigned long long base = 0;
     if (lane == leader) base = atomicAdd(p.count, (unsigned long long)__popc(m));
     base = __shfl_sync(m, base, leader);
     const unsigned long long o = base + __popc(m & ((1u << lane) - 1u));
-    if (o < p.capacity) { p.out_ida[o] = ida; p.out_idb[o] = idb; p.out_sep[o] = sep_from_chord2(c2); }
+    if (o < p.capacity) { p.out_ida[o] = __ldg(A.id + a_row); p.out_idb[o] = __ldg(B.id + b_row); p.out_sep[o] = sep_from_chord2(c2); }
 }
 
 template <int MODE>
-__device__ __forceinline__ void scan_global(const IndexView& B, const MatchArgs& p, long long ida,
+__device__ __forceinline__ void scan_global(const IndexView& A, const IndexView& B, const MatchArgs& p, uint32_t a_row,
                                             double ax, double ay, double az, uint32_t j0, uint32_t j1, Best& h) {
     for (uint32_t j = j0; j < j1; ++j) {
         const double dx = ax - __ldg(B.x + j), dy = ay - __ldg(B.y + j), dz = az - __ldg(B.z + j);
         const double c2 = fma(dx, dx, fma(dy, dy, dz * dz));
         if (c2 <= p.thr2) {
-            const long long idb = __ldg(B.id + j);
-            if (MODE == HLC2_ALL_PAIRS) emit_direct(p, ida, idb, c2);
-            else if (!h.has || c2 < h.c2 || (c2 == h.c2 && idb < h.idb)) { h.has = true; h.idb = idb; h.c2 = c2; }
+            if (MODE == HLC2_ALL_PAIRS) emit_direct(A, B, p, a_row, j, c2);
+            else if (!h.has || c2 < h.c2 || (c2 == h.c2 && __ldg(B.id + j) < __ldg(B.id + h.row))) { h.has = true; h.row = j; h.c2 = c2; }
         }
     }
 }
 
 template <int MODE>
-__device__ __noinline__ void scan_general(const IndexView& B, const MatchArgs& p, long long ida,
+__device__ __noinline__ void scan_general(const IndexView& A, const IndexView& B, const MatchArgs& p, uint32_t a_row,
                                           double ax, double ay, double az, float2 pf, Best& h) {
     const GridView& g = B.g;
     const double dlo = (double)pf.y - p.pad_dec, dhi = (double)pf.y + p.pad_dec;
@@ -349,9 +349,9 @@ __device__ __noinline__ void scan_general(const IndexView& B, const MatchArgs& p
             if (!va) { if (!vx) continue; k0 = k2; k1 = k3; vx = false; }
             if (!vx) k3 = k2 - 1;
         }
-        scan_global<MODE>(B, p, ida, ax, ay, az, __ldg(B.cell_start + base + k0), __ldg(B.cell_start + base + k1 + 1), h);
+        scan_global<MODE>(A, B, p, a_row, ax, ay, az, __ldg(B.cell_start + base + k0), __ldg(B.cell_start + base + k1 + 1), h);
         if (k3 >= k2)
-            scan_global<MODE>(B, p, ida, ax, ay, az, __ldg(B.cell_start + base + k2), __ldg(B.cell_start + base + k3 + 1), h);
+            scan_global<MODE>(A, B, p, a_row, ax, ay, az, __ldg(B.cell_start + base + k2), __ldg(B.cell_start + base + k3 + 1), h);
     }
 }
 
@@ -359,45 +359,46 @@ __device__ __noinline__ void scan_general(const IndexView& B, const MatchArgs& p
 // hit queue of one consumer warp
 // ------------------------------------------------------------------------------------------------------
 // write queue rows [first, first + cnt) to the output: one global atomic, coalesced stores
-__device__ __forceinline__ void flush_rows(const MatchArgs& p, const WarpQueue& q, unsigned first, unsigned cnt, int lane) {
+__device__ __forceinline__ void flush_rows(const IndexView& A, const IndexView& B, const MatchArgs& p, const WarpQueue& q,
+                                           unsigned first, unsigned cnt, int lane) {
     unsigned long long base = 0;
     if (lane == 0) base = atomicAdd(p.count, (unsigned long long)cnt);
     base = __shfl_sync(kFull, base, 0);
     for (unsigned k = lane; k < cnt; k += 32) {
         const unsigned long long o = base + k;
         if (o < p.capacity) {
-            p.out_ida[o] = q.ida[first + k]; p.out_idb[o] = q.idb[first + k];
+            p.out_ida[o] = __ldg(A.id + q.a[first + k]); p.out_idb[o] = __ldg(B.id + q.b[first + k]);
             p.out_sep[o] = sep_from_chord2(q.c2[first + k]);
         }
     }
 }
 
 // append the lanes with `hit`; flush the top kQFlush rows once that many are queued.  qn is warp-uniform.
-__device__ __forceinline__ void push_hits(const MatchArgs& p, WarpQueue& q, unsigned& qn, bool hit,
-                                          long long ida, long long idb, double c2, int lane) {
+__device__ __forceinline__ void push_hits(const IndexView& A, const IndexView& B, const MatchArgs& p, WarpQueue& q, unsigned& qn,
+                                          bool hit, uint32_t a_row, uint32_t b_row, double c2, int lane) {
     const unsigned m = __ballot_sync(kFull, hit);
     if (m == 0) return;
     if (hit) {
         const unsigned k = qn + __popc(m & ((1u << lane) - 1u));
-        q.ida[k] = ida; q.idb[k] = idb; q.c2[k] = c2;
+        q.a[k] = a_row; q.b[k] = b_row; q.c2[k] = c2;
     }
     qn += __popc(m);
     if (qn >= (unsigned)kQFlush) {
         __syncwarp();
         qn -= kQFlush;
-        flush_rows(p, q, qn, kQFlush, lane);
+        flush_rows(A, B, p, q, qn, kQFlush, lane);
         __syncwarp();
     }
 }
 
 // ------------------------------------------------------------------------------------------------------
-// staged scan: every lane tests its rows [p0, p1) of the stage's B arrays; the trip count is the warp's
-// maximum so that hits can be compacted with one ballot per step
+// staged scan: every lane tests its rows [p0, p1) of the stage's B arrays (stage slot j holds B row j - delta); the
+// trip count is the warp's maximum so that hits can be compacted with one ballot per step
 // ------------------------------------------------------------------------------------------------------
 template <int MODE>
-__device__ __forceinline__ void scan_staged(const Stage& st, const MatchArgs& p, WarpQueue& q, unsigned& qn,
-                                            long long ida, double ax, double ay, double az,
-                                            unsigned p0, unsigned p1, Best& best, int lane) {
+__device__ __forceinline__ void scan_staged(const IndexView& A, const IndexView& B, const Stage& st, const MatchArgs& p,
+                                            WarpQueue& q, unsigned& qn, uint32_t a_row, double ax, double ay, double az,
+                                            unsigned p0, unsigned p1, uint32_t delta, Best& best, int lane) {
     const unsigned len = p1 - p0;
     const unsigned mx = __reduce_max_sync(kFull, len);
     // two candidates per step, no branches: a lane past its range reads the sentinel slot, which never matches
@@ -410,27 +411,32 @@ __device__ __forceinline__ void scan_staged(const Stage& st, const MatchArgs& p,
         const double c21 = fma(dx1, dx1, fma(dy1, dy1, dz1 * dz1));
         const bool h0 = c20 <= p.thr2, h1 = c21 <= p.thr2;
         if (MODE == HLC2_ALL_PAIRS) {
-            push_hits(p, q, qn, h0, ida, h0 ? st.bid[j0] : 0ll, c20, lane);
-            push_hits(p, q, qn, h1, ida, h1 ? st.bid[j1] : 0ll, c21, lane);
+            push_hits(A, B, p, q, qn, h0, a_row, j0 - delta, c20, lane);
+            push_hits(A, B, p, q, qn, h1, a_row, j1 - delta, c21, lane);
         } else {
+            // ties -> smaller idB: the ids are only fetched when two candidates are exactly equidistant
             if (h0) {
-                const long long idb = st.bid[j0];
-                if (!best.has || c20 < best.c2 || (c20 == best.c2 && idb < best.idb)) { best.has = true; best.idb = idb; best.c2 = c20; }
+                const uint32_t r = j0 - delta;
+                if (!best.has || c20 < best.c2 || (c20 == best.c2 && __ldg(B.id + r) < __ldg(B.id + best.row))) { best.has = true; best.row = r; best.c2 = c20; }
             }
             if (h1) {
-                const long long idb = st.bid[j1];
-                if (!best.has || c21 < best.c2 || (c21 == best.c2 && idb < best.idb)) { best.has = true; best.idb = idb; best.c2 = c21; }
+                const uint32_t r = j1 - delta;
+                if (!best.has || c21 < best.c2 || (c21 == best.c2 && __ldg(B.id + r) < __ldg(B.id + best.row))) { best.has = true; best.row = r; best.c2 = c21; }
             }
         }
     }
 }
 
+// a lane's up to two row ranges (rows whose Dec window spans two zones) with the slot -> row offsets of their pieces
+struct Ranges { unsigned p0, p1, s0, s1; uint32_t pd, sd; };
+
 // a lane's row ranges in the pieces of a job.  GENERAL: ring and wrap jobs (polar tiles, windows through u = 0 / 360).
 template <int MODE, bool GENERAL>
-__device__ __forceinline__ void seg_ranges(const Stage& st, const MatchArgs& p, WarpQueue& q, unsigned& qn, const GridView& g,
+__device__ __forceinline__ void seg_ranges(const IndexView& A, const IndexView& B, const Stage& st, const MatchArgs& p,
+                                           WarpQueue& q, unsigned& qn, const GridView& g,
                                            uint32_t flags, int nseg, bool act, int zlo, int zhi, double u, double w,
-                                           double vlo0, double vhi0, long long ida, double ax, double ay, double az,
-                                           Best& best, int lane, unsigned& p0, unsigned& p1, unsigned& s0, unsigned& s1) {
+                                           double vlo0, double vhi0, uint32_t a_row, double ax, double ay, double az,
+                                           Best& best, int lane, Ranges& R) {
     const StageDesc& d = st.d;
     for (int sg = 0; sg < nseg; ++sg) {
         const SegDesc& e = d.seg[sg];
@@ -453,12 +459,12 @@ __device__ __forceinline__ void seg_ranges(const Stage& st, const MatchArgs& p, 
         unsigned q0 = st.cs[k0 + e.cdelta], q1 = st.cs[k1 + 1 + e.cdelta];
         q0 = min(max(q0, e.row_lo), e.row_hi) + e.rdelta; q1 = min(max(q1, e.row_lo), e.row_hi) + e.rdelta;
         has = has && q1 > q0;
-        if (sg >= 2 && __any_sync(kFull, has && p1 > p0 && s1 > s0)) {      // a third range: drain first
-            scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, p0, p1, best, lane);
-            scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, s0, s1, best, lane);
-            p0 = p1 = s0 = s1 = 0;
+        if (sg >= 2 && __any_sync(kFull, has && R.p1 > R.p0 && R.s1 > R.s0)) {      // a third range: drain first
+            scan_staged<MODE>(A, B, st, p, q, qn, a_row, ax, ay, az, R.p0, R.p1, R.pd, best, lane);
+            scan_staged<MODE>(A, B, st, p, q, qn, a_row, ax, ay, az, R.s0, R.s1, R.sd, best, lane);
+            R.p0 = R.p1 = R.s0 = R.s1 = 0;
         }
-        if (has) { if (p1 == p0) { p0 = q0; p1 = q1; } else { s0 = q0; s1 = q1; } }
+        if (has) { if (R.p1 == R.p0) { R.p0 = q0; R.p1 = q1; R.pd = e.rdelta; } else { R.s0 = q0; R.s1 = q1; R.sd = e.rdelta; } }
     }
 }
 
@@ -527,10 +533,10 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
             const bool any = nseg != 0 || (flags & kJobDirect);
             const uint32_t a_al = a_first & ~1u;
             const uint32_t a_ld = any ? (((a_first + a_count + 1u) & ~1u) - a_al) : 0u;
-            const uint32_t bytes = a_ld * 40u + rtot * 32u + ctot * 4u;
+            const uint32_t bytes = a_ld * 32u + rtot * 24u + ctot * 4u;
 
             mbar_wait_backoff(&sm.empty[s], ph ^ 1u);
-            if (lane == 0) { st.d.a_count = a_count; st.d.a_off = a_first - a_al; st.d.flags = flags; st.d.nseg = nseg; }
+            if (lane == 0) { st.d.a_first = a_first; st.d.a_count = a_count; st.d.a_off = a_first - a_al; st.d.flags = flags; st.d.nseg = nseg; }
             if (segact) {
                 SegDesc& e = st.d.seg[lane];
                 e.n_d = (double)(int32_t)n_ra; e.centre = (double)__uint_as_float(ctr);
@@ -544,14 +550,13 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
                 bulk_g2s(st.bx + roff, B.x + row_al, n_ld * 8u, &sm.full[s]);
                 bulk_g2s(st.by + roff, B.y + row_al, n_ld * 8u, &sm.full[s]);
                 bulk_g2s(st.bz + roff, B.z + row_al, n_ld * 8u, &sm.full[s]);
-                bulk_g2s(st.bid + roff, B.id + row_al, n_ld * 8u, &sm.full[s]);
                 bulk_g2s(st.cs + coff, B.cell_start + cs_al, c_ld * 4u, &sm.full[s]);
             }
-            if (a_ld && lane >= 8 && lane < 13) {
+            if (a_ld && lane >= 8 && lane < 12) {
                 const int k = lane - 8;
                 const void* src = k == 0 ? (const void*)(A.x + a_al) : k == 1 ? (const void*)(A.y + a_al) : k == 2 ? (const void*)(A.z + a_al)
-                                : k == 3 ? (const void*)(A.pos + a_al) : (const void*)(A.id + a_al);
-                void* dst = k == 0 ? (void*)st.ax : k == 1 ? (void*)st.ay : k == 2 ? (void*)st.az : k == 3 ? (void*)st.apos : (void*)st.aid;
+                                : (const void*)(A.pos + a_al);
+                void* dst = k == 0 ? (void*)st.ax : k == 1 ? (void*)st.ay : k == 2 ? (void*)st.az : (void*)st.apos;
                 bulk_g2s(dst, src, a_ld * 8u, &sm.full[s]);
             }
             wcur = wnext; have = nhave;
@@ -567,7 +572,7 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
     const GridView& g = B.g;
     WarpQueue& q = sm.q[warp];
     unsigned qn = 0;
-    Best best; best.has = false; best.c2 = 0.0; best.idb = 0;
+    Best best; best.has = false; best.c2 = 0.0; best.row = 0;
     for (uint32_t it = 0;; ++it) {
         const int s = (int)(it % kStages);
         const unsigned ph = (it / kStages) & 1u;
@@ -584,14 +589,13 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
 #endif
             const bool act = threadIdx.x < a_count;
             if (MODE == HLC2_NEAREST && (flags & kJobFirst)) best.has = false;
-            long long ida = 0;
+            const uint32_t a_row = d.a_first + threadIdx.x;
             if (nseg != 0 || (flags & kJobDirect)) {
                 const unsigned ra = act ? threadIdx.x + d.a_off : d.a_off;
                 const double ax = st.ax[ra], ay = st.ay[ra], az = st.az[ra];
                 const float2 pf = st.apos[ra];
-                ida = st.aid[ra];
                 if (flags & kJobDirect) {
-                    if (act) scan_general<MODE>(B, p, ida, ax, ay, az, pf, best);
+                    if (act) scan_general<MODE>(A, B, p, a_row, ax, ay, az, pf, best);
                     __syncwarp();
                 } else {
                     const double dlo = (double)pf.y - p.pad_dec, dhi = (double)pf.y + p.pad_dec;
@@ -601,25 +605,22 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
                     const double w = (double)(sn * (1.011f * 57.29577951f)) + kEpsRaDeg;
                     const double u = box_u(g, (double)pf.x);
                     const double vlo0 = (u - w) * g.inv_span, vhi0 = (u + w) * g.inv_span;
-                    unsigned p0 = 0, p1 = 0, s0 = 0, s1 = 0;      // a lane's first and (zone-spanning rows) second range
+                    Ranges R; R.p0 = R.p1 = R.s0 = R.s1 = 0; R.pd = R.sd = 0;
                     if (flags & (kJobRing | kJobWrap))
-                        seg_ranges<MODE, true>(st, p, q, qn, g, flags, nseg, act, zlo, zhi, u, w, vlo0, vhi0, ida, ax, ay, az, best, lane, p0, p1, s0, s1);
+                        seg_ranges<MODE, true>(A, B, st, p, q, qn, g, flags, nseg, act, zlo, zhi, u, w, vlo0, vhi0, a_row, ax, ay, az, best, lane, R);
                     else
-                        seg_ranges<MODE, false>(st, p, q, qn, g, flags, nseg, act, zlo, zhi, u, w, vlo0, vhi0, ida, ax, ay, az, best, lane, p0, p1, s0, s1);
-                    scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, p0, p1, best, lane);
-                    if (__any_sync(kFull, s1 > s0)) scan_staged<MODE>(st, p, q, qn, ida, ax, ay, az, s0, s1, best, lane);
+                        seg_ranges<MODE, false>(A, B, st, p, q, qn, g, flags, nseg, act, zlo, zhi, u, w, vlo0, vhi0, a_row, ax, ay, az, best, lane, R);
+                    scan_staged<MODE>(A, B, st, p, q, qn, a_row, ax, ay, az, R.p0, R.p1, R.pd, best, lane);
+                    if (__any_sync(kFull, R.s1 > R.s0)) scan_staged<MODE>(A, B, st, p, q, qn, a_row, ax, ay, az, R.s0, R.s1, R.sd, best, lane);
                 }
             }
-            if (MODE == HLC2_NEAREST && (flags & kJobLast)) {
-                if (nseg == 0 && !(flags & kJobDirect)) ida = st.aid[act ? threadIdx.x + d.a_off : d.a_off];
-                push_hits(p, q, qn, act && best.has, ida, best.idb, best.c2, lane);
-            }
+            if (MODE == HLC2_NEAREST && (flags & kJobLast)) push_hits(A, B, p, q, qn, act && best.has, a_row, best.row, best.c2, lane);
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm.empty[s]);
     }
     __syncwarp();
-    if (qn) flush_rows(p, q, 0, qn, lane);
+    if (qn) flush_rows(A, B, p, q, 0, qn, lane);
 }
 
 static inline size_t pool_cap_of(size_t tile_cap) { return 3 * tile_cap + 4096; }
