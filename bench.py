@@ -159,6 +159,7 @@ def main():
     ap.add_argument("--sample-ra-deg", type=float, default=108.0, help="RA slice of the CPU-baseline sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--occupancy", type=float, default=0.0)
+    ap.add_argument("--occupancy-b", type=float, default=None, help="target occupancy of B's index (default: same as --occupancy)")
     ap.add_argument("--bands", type=int, default=16, help="declination bands of the streamed e2e leg")
     ap.add_argument("--no-stream", action="store_true", help="skip the streamed e2e leg")
     args = ap.parse_args()
@@ -195,7 +196,7 @@ def main():
     dA = [t.cuda(non_blocking=True) for t in hA]; dB = [t.cuda(non_blocking=True) for t in hB]
     torch.cuda.synchronize()
 
-    opts_a = P.make_opts(r, target_occupancy=args.occupancy); opts_b = P.make_opts(r, target_occupancy=args.occupancy)
+    opts_a = P.make_opts(r, target_occupancy=args.occupancy); opts_b = P.make_opts(r, target_occupancy=args.occupancy if args.occupancy_b is None else args.occupancy_b)
     ib_a, tb_a = P.hlc2_index_sizes(n_a, opts_a); ib_b, tb_b = P.hlc2_index_sizes(n_b, opts_b)
     buf_a = torch.empty(ib_a, dtype=torch.uint8, device="cuda"); buf_b = torch.empty(ib_b, dtype=torch.uint8, device="cuda")
     temp = torch.empty(max(tb_a, tb_b), dtype=torch.uint8, device="cuda")
