@@ -351,27 +351,44 @@ k_cell_fill(const uint32_t* __restrict__ keys, uint32_t n, uint32_t n_cells, uin
             uint32_t* __restrict__ big, uint32_t* __restrict__ big_count, uint32_t big_cap) {
     const int lane = threadIdx.x & 31;
     const size_t total = (size_t)n + 1;
-    const size_t stride = (size_t)gridDim.x * 256;
-    for (size_t b = (size_t)blockIdx.x * 256 + (threadIdx.x & ~31); b < total; b += stride) {   // warp-uniform trip count
-        const size_t i = b + lane;
-        uint32_t lo = 1, hi = 0;                           // empty
-        if (i < total) {
-            hi = i < n ? __ldg(keys + i) : n_cells;
-            lo = i > 0 ? __ldg(keys + i - 1) + 1u : 0u;
-            if (i > 0 && i < n && hi + 1u == lo) { lo = 1; hi = 0; }      // same cell as the previous row
+    // a warp takes 128 consecutive rows per step, four per lane (one 16-byte load): a pass that moves 4 bytes per
+    // row needs that many bytes in flight to cover the DRAM latency
+    const size_t stride = (size_t)gridDim.x * 256 * 4;
+    for (size_t b = ((size_t)blockIdx.x * 256 + (threadIdx.x & ~31)) * 4; b < total; b += stride) {   // warp-uniform trip count
+        const size_t i0 = b + 4 * (size_t)lane;
+        uint32_t k[4];
+        if (i0 + 3 < n) {
+            const uint4 v = __ldg(reinterpret_cast<const uint4*>(keys + i0));
+            k[0] = v.x; k[1] = v.y; k[2] = v.z; k[3] = v.w;
+        } else {
+#pragma unroll
+            for (int j = 0; j < 4; ++j) k[j] = i0 + j < n ? __ldg(keys + i0 + j) : n_cells;
         }
-        const uint32_t span = hi >= lo ? hi - lo + 1u : 0u;
-        if (span && span <= kFillLane) for (uint32_t c = lo; c <= hi; ++c) cell_start[c] = (uint32_t)i;
-        unsigned m = __ballot_sync(0xffffffffu, span > kFillLane);
-        while (m) {
-            const int src = __ffs(m) - 1; m &= m - 1;
-            const uint32_t l = __shfl_sync(0xffffffffu, lo, src), h = __shfl_sync(0xffffffffu, hi, src);
-            const uint32_t v = (uint32_t)(b + src);
-            if (h - l + 1u <= kFillWarp) {
-                for (uint64_t cc = (uint64_t)l + lane; cc <= h; cc += 32) cell_start[cc] = v;
-            } else if (lane == 0) {
-                uint32_t e = atomicAdd(big_count, 1u);
-                if (e < big_cap) { big[3 * e] = l; big[3 * e + 1] = h; big[3 * e + 2] = v; }
+        uint32_t prev = __shfl_up_sync(0xffffffffu, k[3], 1);
+        if (lane == 0) prev = b > 0 ? __ldg(keys + b - 1) : 0u;
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const size_t i = i0 + j;
+            uint32_t lo = 1, hi = 0;                           // empty
+            if (i < total) {
+                hi = k[j];                                     // row n (one past the end) closes every cell above key[n-1]
+                lo = i > 0 ? prev + 1u : 0u;
+                if (i > 0 && i < n && hi + 1u == lo) { lo = 1; hi = 0; }      // same cell as the previous row
+            }
+            prev = k[j];
+            const uint32_t span = hi >= lo ? hi - lo + 1u : 0u;
+            if (span && span <= kFillLane) for (uint32_t c = lo; c <= hi; ++c) cell_start[c] = (uint32_t)i;
+            unsigned m = __ballot_sync(0xffffffffu, span > kFillLane);
+            while (m) {
+                const int src = __ffs(m) - 1; m &= m - 1;
+                const uint32_t l = __shfl_sync(0xffffffffu, lo, src), h = __shfl_sync(0xffffffffu, hi, src);
+                const uint32_t v = (uint32_t)(b + 4 * (size_t)src + j);
+                if (h - l + 1u <= kFillWarp) {
+                    for (uint64_t cc = (uint64_t)l + lane; cc <= h; cc += 32) cell_start[cc] = v;
+                } else if (lane == 0) {
+                    uint32_t e = atomicAdd(big_count, 1u);
+                    if (e < big_cap) { big[3 * e] = l; big[3 * e + 1] = h; big[3 * e + 2] = v; }
+                }
             }
         }
     }
@@ -394,7 +411,7 @@ void launch_cell_table(const uint32_t* sorted_keys, uint32_t n, uint32_t n_cells
     const uint32_t cap = (uint32_t)cell_big_cap(n_cells);
     uint32_t* d_count = d_big + 3 * (size_t)cap;
     cudaMemsetAsync(d_count, 0, sizeof(uint32_t), s);
-    int blocks = (int)std::min<size_t>(((size_t)n + 1 + 255) / 256, (size_t)sm_count() * 16);
+    int blocks = (int)std::min<size_t>(((size_t)n + 1 + 1023) / 1024, (size_t)sm_count() * 16);
     k_cell_fill<<<blocks, 256, 0, s>>>(sorted_keys, n, n_cells, cell_start, d_big, d_count, cap); count_launch();
     k_cell_fill_big<<<sm_count() * 4, 256, 0, s>>>(d_big, d_count, cap, cell_start); count_launch();
 }
