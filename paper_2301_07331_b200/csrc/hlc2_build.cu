@@ -349,7 +349,9 @@ constexpr uint32_t kFillLane = 4, kFillWarp = 4096;
 __global__ void __launch_bounds__(256)
 k_cell_fill(const uint32_t* __restrict__ keys, uint32_t n, uint32_t n_cells, uint32_t* __restrict__ cell_start,
             uint32_t* __restrict__ big, uint32_t* __restrict__ big_count, uint32_t big_cap) {
+    __shared__ uint32_t s_keys[8][128];
     const int lane = threadIdx.x & 31;
+    uint32_t* sk = s_keys[threadIdx.x >> 5];
     const size_t total = (size_t)n + 1;
     // a warp takes 128 consecutive rows per step, four per lane (one 16-byte load): a pass that moves 4 bytes per
     // row needs that many bytes in flight to cover the DRAM latency
@@ -366,6 +368,31 @@ k_cell_fill(const uint32_t* __restrict__ keys, uint32_t n, uint32_t n_cells, uin
         }
         uint32_t prev = __shfl_up_sync(0xffffffffu, k[3], 1);
         if (lane == 0) prev = b > 0 ? __ldg(keys + b - 1) : 0u;
+        // common case, no long empty run inside the 128 rows: lanes own CELLS, not rows -- cell c gets the first row of
+        // the step whose key is >= c (a binary search over the step's keys in shared memory), so the stores of a warp
+        // are consecutive words instead of scattered ones
+        {
+            uint32_t p = prev;
+            bool longrun = false;
+#pragma unroll
+            for (int j = 0; j < 4; ++j) { longrun |= k[j] - p > kFillWarp && i0 + j < total && (i0 + j > 0); p = k[j]; }
+            if (!__any_sync(0xffffffffu, longrun)) {
+                const uint32_t lo_cell = b > 0 ? __shfl_sync(0xffffffffu, prev, 0) + 1u : 0u;
+                const uint32_t hi_cell = __shfl_sync(0xffffffffu, k[3], 31);
+                __syncwarp();
+                sk[4 * lane] = k[0]; sk[4 * lane + 1] = k[1]; sk[4 * lane + 2] = k[2]; sk[4 * lane + 3] = k[3];
+                __syncwarp();
+                if (hi_cell >= lo_cell && hi_cell - lo_cell <= 32u * kFillWarp) {
+                    for (uint64_t c = (uint64_t)lo_cell + lane; c <= hi_cell; c += 32) {
+                        uint32_t pos = 0;
+#pragma unroll
+                        for (int st = 64; st >= 1; st >>= 1) if (sk[pos + st - 1] < (uint32_t)c) pos += st;
+                        cell_start[c] = (uint32_t)(b + pos);
+                    }
+                    continue;
+                }
+            }
+        }
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const size_t i = i0 + j;
