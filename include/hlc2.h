@@ -68,7 +68,8 @@ typedef enum {
  *   r_max_arcsec      largest radius the index will be queried with; > 0, <= 36000 (10 deg).
  *                     Fine cells are never smaller than this ("cells sized to r", NS (a)), so a
  *                     search window spans at most 3 zones.
- *   target_occupancy  mean sources per fine cell over the occupied sky; 0 -> 1.0.
+ *   target_occupancy  mean sources per fine cell over the occupied sky; 0 -> automatic: the finest value in
+ *                     [0.5, 1] whose cell count needs no more radix-sort digits than occupancy 1 would.
  *   cell_arcsec       explicit fine-cell size; 0 -> derived from the catalogue's density
  *                     (max(r_max, sqrt(target_occupancy * occupied area / n))).  Honoured while the cell
  *                     table stays within max(16 n, 2^25) cells, else coarsened until it fits.

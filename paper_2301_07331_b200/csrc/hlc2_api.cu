@@ -66,10 +66,21 @@ static bool opts_ok(const hlc2_opts* o) {
     if (o->grid_like && o->grid_like->magic != kMagic) return false;
     return true;
 }
-static hlc2_opts opts_or_default(const hlc2_opts* o) {
+// target_occupancy 0 = automatic: cells as fine as the radix sort allows for free.  Finer cells of the scanned
+// catalogue mean fewer candidates per source in the match (config 3: occupancy 0.5 instead of 1 takes 7 % off the match),
+// but a cell count that needs one more key digit costs a whole extra sort pass in the build; so take the finest
+// occupancy in [0.5, 1] whose cell count still fits the digits that occupancy 1 needs.
+static double auto_occupancy(int64_t n) {
+    if (n <= 0) return 1.0;
+    int bits = 1; while (bits < 32 && (1ull << bits) < (unsigned long long)n) ++bits;      // key bits at occupancy 1
+    const int passes = std::max(1, (bits + kRadixBits - 1) / kRadixBits);
+    const double max_cells = std::ldexp(1.0, std::min(32, passes * kRadixBits));
+    return std::min(1.0, std::max(0.5, 1.15 * (double)n / max_cells));
+}
+static hlc2_opts opts_or_default(const hlc2_opts* o, int64_t n) {
     hlc2_opts d; memset(&d, 0, sizeof d); d.r_max_arcsec = 1.0;
     if (o) d = *o;
-    if (d.target_occupancy == 0.0) d.target_occupancy = 1.0;
+    if (d.target_occupancy == 0.0) d.target_occupancy = auto_occupancy(n);
     if (d.target_occupancy < 0.05) d.target_occupancy = 0.05;
     return d;
 }
@@ -132,7 +143,7 @@ static TempLayout make_temp(int64_t n, const Layout& L) {
 
 namespace hlc2 {
 size_t match_temp_bound(int64_t n_a, const hlc2_opts* opts) {
-    hlc2_opts o = opts_or_default(opts);
+    hlc2_opts o = opts_or_default(opts, n_a);
     o.grid_like = nullptr;
     Layout L = make_layout(n_a, o);
     return match_temp_for_tiles(L.cap_tiles);
@@ -239,7 +250,7 @@ extern "C" {
 int hlc2_index_sizes(int64_t n, const hlc2_opts* opts, size_t* index_bytes, size_t* temp_bytes) {
     if (n < 0 || !opts_ok(opts) || (!index_bytes && !temp_bytes)) return HLC2_ERR_INVALID_ARG;
     if ((uint64_t)n > kMaxN) return HLC2_ERR_TOO_MANY;
-    hlc2_opts o = opts_or_default(opts);
+    hlc2_opts o = opts_or_default(opts, n);
     Layout L = make_layout(n, o);
     TempLayout T = make_temp(n, L);
     if (index_bytes) *index_bytes = L.total;
@@ -254,7 +265,7 @@ int hlc2_build_index(const double* d_ra, const double* d_dec, const int64_t* d_i
     *out = nullptr;
     if (n < 0 || !opts_ok(opts) || !d_index_buf || !d_temp || (n > 0 && (!d_ra || !d_dec))) return HLC2_ERR_INVALID_ARG;
     if ((uint64_t)n > kMaxN) return HLC2_ERR_TOO_MANY;
-    hlc2_opts o = opts_or_default(opts);
+    hlc2_opts o = opts_or_default(opts, n);
     Layout L = make_layout(n, o);
     TempLayout T = make_temp(n, L);
     if (index_bytes < L.total || temp_bytes < T.total) return HLC2_ERR_BUFFER_TOO_SMALL;
