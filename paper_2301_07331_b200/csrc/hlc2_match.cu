@@ -45,7 +45,7 @@ constexpr int kMatchThreads = kTile + 32;    // + the producer warp
 #define HLC2_BCAP 320
 #endif
 #ifndef HLC2_CSCAP
-#define HLC2_CSCAP 768
+#define HLC2_CSCAP 1024
 #endif
 #ifndef HLC2_QCAP
 #define HLC2_QCAP 64
