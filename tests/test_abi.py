@@ -93,3 +93,16 @@ def test_product_has_no_cpu_fallback(P):
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 txt = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in txt and "from oracle" not in txt and "hlc2_oracle" not in txt
+
+
+def test_size_queries_grow_with_n(P):
+    """hlc2_stream_crossmatch sizes its arena for the largest band and builds smaller ones inside it: the size queries
+    must never shrink when n grows (also across the automatic-occupancy brackets)."""
+    import numpy as np
+    o = P.make_opts(1.0)
+    ns = sorted({int(x) for x in np.concatenate([np.arange(1, 2000), np.logspace(3.3, 8.9, 1500)])})
+    prev = (0, 0)
+    for n in ns:
+        cur = P.hlc2_index_sizes(n, o)
+        assert cur[0] >= prev[0] and cur[1] >= prev[1], (n, cur, prev)
+        prev = cur
