@@ -87,18 +87,39 @@ void launch_stats(const double* ra, const double* dec, uint32_t n, Stats* d_stat
 // exact), Dec uses the colatitude 90 - |dec| (exact) beyond 45 deg, so the radian conversion never rounds an
 // angle larger than pi/4; unit-vector chords are then good to ~5e-11 arcsec.
 // ------------------------------------------------------------------------------------------
+// sin and cos of |x| <= pi/4 without range reduction: the classic minimax polynomials of that interval (Cephes
+// sin.c / cos.c coefficients; |error| < 1.2e-16, sin keeps full relative accuracy for tiny x).  The arguments here are
+// already reduced in the degree domain, so the library sincos' reduction and special cases are dead weight.
+__device__ __forceinline__ void sincos_quarter(double x, double& s, double& c) {
+    const double z = x * x;
+    double ps = 1.58962301576546568060e-10;
+    ps = fma(ps, z, -2.50507477628578072866e-8);
+    ps = fma(ps, z, 2.75573136213857245213e-6);
+    ps = fma(ps, z, -1.98412698295895385996e-4);
+    ps = fma(ps, z, 8.33333333332211858878e-3);
+    ps = fma(ps, z, -1.66666666666666307295e-1);
+    s = fma(x * z, ps, x);
+    double pc = -1.13585365213876817300e-11;
+    pc = fma(pc, z, 2.08757008419747316778e-9);
+    pc = fma(pc, z, -2.75573141792967388112e-7);
+    pc = fma(pc, z, 2.48015872888517045348e-5);
+    pc = fma(pc, z, -1.38888888888730564116e-3);
+    pc = fma(pc, z, 4.16666666666665929218e-2);
+    c = fma(z * z, pc, fma(-0.5, z, 1.0));
+}
+
 __device__ __forceinline__ void unit_vector(double ra_norm, double dec, double& x, double& y, double& z) {
     const double D2R = 0.017453292519943295;   // pi / 180
     double q = rint(ra_norm * (1.0 / 90.0));
     double t = fma(-90.0, q, ra_norm);
-    double st, ct; sincos(t * D2R, &st, &ct);
+    double st, ct; sincos_quarter(t * D2R, st, ct);
     int iq = ((int)q) & 3;
     double ca = (iq == 0) ? ct : (iq == 1) ? -st : (iq == 2) ? -ct : st;
     double sa = (iq == 0) ? st : (iq == 1) ? ct : (iq == 2) ? -st : -ct;
-    double ad = fabs(dec), sd, cd;
-    if (ad > 45.0) { double s, c; sincos((90.0 - ad) * D2R, &s, &c); sd = c; cd = s; }
-    else           { sincos(ad * D2R, &sd, &cd); }
-    sd = copysign(sd, dec);
+    const double ad = fabs(dec);
+    const bool polar = ad > 45.0;
+    double s, c; sincos_quarter((polar ? 90.0 - ad : ad) * D2R, s, c);
+    const double sd = copysign(polar ? c : s, dec), cd = polar ? s : c;
     x = cd * ca; y = cd * sa; z = sd;
 }
 
