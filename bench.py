@@ -246,6 +246,16 @@ def main():
     ph = np.array([[m[0].elapsed_time(m[1]), m[1].elapsed_time(m[2]), m[2].elapsed_time(m[3])] for m in marks])
     t_build_a, t_build_b, t_match = ph.mean(axis=0)
 
+    # ---- the dominant kernel alone: CUDA events recorded by the library around k_match on this stream (the planner and
+    # the count memset of the hlc2_crossmatch call are left out), one launch at a time on the indices of the last step ----
+    P.hlc2_time_match_kernel(True)
+    kms = []
+    for _ in range(max(5, args.steps)):
+        P.hlc2_crossmatch(ia, ib, r, mode, out_a, out_b, out_s, cnt, temp=temp)
+        kms.append(P.hlc2_last_match_kernel_ms())
+    P.hlc2_time_match_kernel(False)
+    t_kernel = float(np.mean(kms))
+
     # ---- timed region 2 (e2e): host buffers, H2D of the inputs and D2H of the results inside the region ----
     def e2e_step():
         da = [t.cuda(non_blocking=True) for t in hA]; db = [t.cuda(non_blocking=True) for t in hB]
@@ -309,12 +319,15 @@ def main():
     if rank == 0:
         peak, peak_src = peak_hbm()
         alg_bytes = 32.0 * n_a + 32.0 * n_b + 24.0 * found          # catalogue (sorted SoA) + output bytes
-        achieved = alg_bytes / (t_match * 1e-3) / 1e9
+        achieved = alg_bytes / (t_kernel * 1e-3) / 1e9
         tr = ncu_traffic()
-        roof = {"bound": "hbm", "kernel": "k_match (timed as the whole hlc2_crossmatch call: count memset + k_plan + k_match)", "achieved": achieved, "peak": peak, "unit": "GB/s",
+        roof = {"bound": "hbm", "kernel": "k_match", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0, "peak_source": peak_src,
                 "traffic": tr["dram_bytes_per_launch"] if tr else None, "algorithmic_bytes": alg_bytes,
-                "ms_per_launch": float(t_match)}
+                "ms_per_launch": t_kernel, "launches_timed": len(kms),
+                "timing": "CUDA events recorded by the library around k_match on the caller's stream (hlc2_time_match_kernel)",
+                "whole_call": {"ms": float(t_match), "frac": alg_bytes / (t_match * 1e-3) / 1e9 / peak,
+                               "what": "hlc2_crossmatch inside the timed steps: count memset + k_plan + k_match"}}
         cpu = None
         if not args.no_cpu_baseline:
             sa, sb = sample_patch(w, 0.0, args.sample_ra_deg)

@@ -197,6 +197,11 @@ const char* hlc2_strerror(int status);
 int hlc2_last_cuda_error(const char** message);
 /* Number of kernels this library has launched since it was loaded (for launch accounting). */
 unsigned long long hlc2_kernel_launches(void);
+/* Measurement hook: when enabled, hlc2_crossmatch brackets its match kernel (not the planner) with CUDA events on the
+ * caller's stream; hlc2_last_match_kernel_ms waits for the latest such launch and returns its duration in *ms
+ * (HLC2_ERR_INVALID_ARG if none was timed).  Process-wide, not thread-safe; off by default. */
+int hlc2_time_match_kernel(int enable);
+int hlc2_last_match_kernel_ms(float* ms);
 const char* hlc2_version(void);
 
 #ifdef __cplusplus

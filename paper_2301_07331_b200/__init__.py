@@ -80,6 +80,8 @@ def lib():
         L.hlc2_strerror.restype = ctypes.c_char_p
         L.hlc2_last_cuda_error.argtypes = [P(ctypes.c_char_p)]
         L.hlc2_kernel_launches.restype = ctypes.c_ulonglong
+        L.hlc2_time_match_kernel.argtypes = [ctypes.c_int]
+        L.hlc2_last_match_kernel_ms.argtypes = [P(ctypes.c_float)]
         L.hlc2_version.restype = ctypes.c_char_p
         _lib = L
     return _lib
@@ -278,6 +280,18 @@ def hlc2_stream_crossmatch(a_cols, a_off, b_cols, b_off, band_edges_deg, radius_
         e = Hlc2Error(rc, "hlc2_stream_crossmatch"); e.found = cnt.value
         raise e
     return int(cnt.value)
+
+def hlc2_time_match_kernel(enable: bool) -> None:
+    lib().hlc2_time_match_kernel(1 if enable else 0)
+
+
+def hlc2_last_match_kernel_ms() -> float:
+    ms = ctypes.c_float(0.0)
+    rc = lib().hlc2_last_match_kernel_ms(ctypes.byref(ms))
+    if rc != HLC2_OK:
+        raise Hlc2Error(rc, "hlc2_last_match_kernel_ms")
+    return float(ms.value)
+
 
 def kernel_launches() -> int:
     return int(lib().hlc2_kernel_launches())

@@ -425,6 +425,10 @@ int hlc2_last_cuda_error(const char** message) {
 
 unsigned long long hlc2_kernel_launches(void) { return hlc2::g_launches.load(std::memory_order_relaxed); }
 
+int hlc2_time_match_kernel(int enable) { hlc2::set_time_match(enable != 0); return HLC2_OK; }
+
+int hlc2_last_match_kernel_ms(float* ms) { return hlc2::last_match_ms(ms); }
+
 const char* hlc2_version(void) { return "hlc2-b200 0.1 (sm_100a)"; }
 
 }  // extern "C"

@@ -92,6 +92,9 @@ void launch_match(const IndexView& A, const IndexView& B, double radius_arcsec, 
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
                   unsigned long long* d_count, void* d_temp, cudaStream_t s);
 
+void set_time_match(bool on);
+int last_match_ms(float* ms);
+
 void count_launch(int k = 1);
 
 }  // namespace hlc2

@@ -623,6 +623,9 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
     if (qn) flush_rows(A, B, p, q, 0, qn, lane);
 }
 
+static bool g_time_match = false, g_match_timed = false;
+static cudaEvent_t g_match_ev[2] = {nullptr, nullptr};
+
 static inline size_t pool_cap_of(size_t tile_cap) { return 3 * tile_cap + 4096; }
 
 size_t match_temp_for_tiles(size_t tile_cap) { return (tile_cap + pool_cap_of(tile_cap)) * sizeof(Job) + 256; }
@@ -673,9 +676,21 @@ void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_ar
     count_launch();
     // persistent grid: SM count x resident CTAs, never more CTAs than tiles
     const unsigned blocks = (unsigned)std::max<size_t>(1, std::min<size_t>(tiles, (size_t)sm_count() * per_sm[m]));
+    if (g_time_match) {                      // measurement hook (hlc2_time_match_kernel): events around k_match alone
+        if (!g_match_ev[0]) { cudaEventCreate(&g_match_ev[0]); cudaEventCreate(&g_match_ev[1]); }
+        cudaEventRecord(g_match_ev[0], s);
+    }
     if (m) k_match<HLC2_NEAREST><<<blocks, kMatchThreads, smem, s>>>(A, B, p);
     else   k_match<HLC2_ALL_PAIRS><<<blocks, kMatchThreads, smem, s>>>(A, B, p);
     count_launch();
+    if (g_time_match) { cudaEventRecord(g_match_ev[1], s); g_match_timed = true; }
+}
+
+void set_time_match(bool on) { g_time_match = on; }
+int last_match_ms(float* ms) {
+    if (!g_match_timed || !ms) return HLC2_ERR_INVALID_ARG;
+    if (cudaEventSynchronize(g_match_ev[1]) != cudaSuccess || cudaEventElapsedTime(ms, g_match_ev[0], g_match_ev[1]) != cudaSuccess) return HLC2_ERR_CUDA;
+    return HLC2_OK;
 }
 
 }  // namespace hlc2

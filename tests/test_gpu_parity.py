@@ -268,3 +268,16 @@ def test_launch_counter_moves(P):
     n0 = P.kernel_launches()
     gpu_match(P, w.A, w.B, 1.0, 0)
     assert P.kernel_launches() - n0 >= 10
+
+
+def test_match_kernel_timing_hook(P):
+    """hlc2_time_match_kernel brackets k_match with events on the caller's stream; results are unaffected."""
+    w = S.config(1, scale=0.3)
+    ga, gb, gs, ia, ib = gpu_match(P, w.A, w.B, w.radius_arcsec, 0)
+    P.hlc2_time_match_kernel(True)
+    try:
+        a, b, s = P.crossmatch(ia, ib, w.radius_arcsec, 0)
+        ms = P.hlc2_last_match_kernel_ms()
+    finally:
+        P.hlc2_time_match_kernel(False)
+    assert 0.0 < ms < 50.0 and len(a) == len(ga)
