@@ -100,7 +100,9 @@ typedef struct {
 
 /* Upper bounds, for `n` sources and these options, of the index buffer and of the build's
  * temporary buffer (both 256-byte aligned device memory).  opts may be NULL (defaults with
- * r_max = 1 arcsec). */
+ * r_max = 1 arcsec).  The role of the paper's source-reading module, which queries free CPU / GPU
+ * memory before cutting calculation blocks (Eq. (8)-(9) P:L259-263): here the caller owns the
+ * memory and asks how much a catalogue of n records needs (NS: "PyTorch used only for device memory"). */
 int hlc2_index_sizes(int64_t n, const hlc2_opts* opts, size_t* index_bytes, size_t* temp_bytes);
 
 /*
@@ -114,7 +116,9 @@ int hlc2_index_sizes(int64_t n, const hlc2_opts* opts, size_t* index_bytes, size
  *   d_temp               scratch of >= temp_bytes; free to reuse when the stream has drained.
  *   out                  receives the handle.
  * Bad coordinates do not fail the build (it is asynchronous): they are recorded and
- * reported by hlc2_index_status; matching against such an index is undefined but safe.
+ * reported by hlc2_index_status.  Such rows are kept in the index with a NaN unit vector, which no
+ * chord test can pass: they never appear in a result, neither as idA nor as idB; all other rows are
+ * matched as usual.
  * The inputs are not modified and are not referenced after the build's work completes.
  */
 int hlc2_build_index(const double* d_ra_deg, const double* d_dec_deg, const int64_t* d_id, int64_t n,
@@ -122,7 +126,9 @@ int hlc2_build_index(const double* d_ra_deg, const double* d_dec_deg, const int6
                      void* d_temp, size_t temp_bytes, void* cuda_stream, hlc2_index** out);
 
 /* Synchronises the build stream.  Returns HLC2_OK, or HLC2_ERR_BAD_COORD with the smallest
- * offending row in *first_bad_row (may be NULL). */
+ * offending row in *first_bad_row (may be NULL).  A catalogue is a table of (RA, Dec) positions in
+ * degrees (Table 2); a non-finite value or |Dec| > 90 is not a position, and the
+ * paper's extraction module would have dropped such a record before the kernel saw it. */
 int hlc2_index_status(const hlc2_index* idx, int64_t* first_bad_row);
 
 /* Grid description.  *h_n_ra (may be NULL) receives a host pointer to n_zones int32 values
@@ -141,7 +147,9 @@ int hlc2_index_arrays(const hlc2_index* idx, const double** d_x, const double** 
                       const int64_t** d_id, const uint32_t** d_cell_start, const uint32_t** d_cell_key,
                       int64_t* n, int64_t* n_cells);
 
-/* Scratch needed by hlc2_crossmatch for this pair of indices (may be 0). */
+/* Scratch needed by hlc2_crossmatch for this pair of indices (may be 0): the job records into which the
+ * planner cuts every A tile's window -- the role of the paper's calculation blocks, whose
+ * memory the paper's tool sized itself (Eq. (8)-(9)) and the caller sizes here. */
 int hlc2_crossmatch_sizes(const hlc2_index* A, const hlc2_index* B, size_t* temp_bytes);
 
 /*
@@ -159,6 +167,16 @@ int hlc2_crossmatch(const hlc2_index* A, const hlc2_index* B, double radius_arcs
                     int64_t* d_out_idA, int64_t* d_out_idB, double* d_out_sep_arcsec,
                     int64_t capacity, unsigned long long* d_count,
                     void* d_temp, size_t temp_bytes, void* cuda_stream);
+
+/* hlc2_crossmatch with two caller-owned CUDA events (cudaEvent_t passed as void*, either may be NULL) that the
+ * call records on cuda_stream immediately before and after the match kernel itself, leaving the planner and the
+ * count memset outside: the measurement NS asks for ("the matching phase" against the HBM roofline).  No state is
+ * kept in the library; the caller reads the events. */
+int hlc2_crossmatch_events(const hlc2_index* A, const hlc2_index* B, double radius_arcsec, int mode,
+                           int64_t* d_out_idA, int64_t* d_out_idB, double* d_out_sep_arcsec,
+                           int64_t capacity, unsigned long long* d_count,
+                           void* d_temp, size_t temp_bytes, void* cuda_stream,
+                           void* ev_kernel_start, void* ev_kernel_stop);
 
 /*
  * Partition streaming from pinned host memory (NS (c); the paper's pinned
@@ -191,17 +209,16 @@ int hlc2_stream_crossmatch(const double* h_a_ra, const double* h_a_dec, const in
                            int64_t* h_out_idA, int64_t* h_out_idB, double* h_out_sep_arcsec, int64_t capacity,
                            unsigned long long* h_count, void* d_arena, size_t arena_bytes, int64_t max_band_out);
 
+/* Releases the handle's host metadata (the device buffers are the caller's; NS: "PyTorch used only for
+ * device memory and streams").  NULL is ignored. */
 void hlc2_index_destroy(hlc2_index* idx);
+/* Text of a status code of this interface (the paper's tool is a CLI that reports on the console, P:L100;
+ * a library reports through codes). */
 const char* hlc2_strerror(int status);
 /* The last cudaError_t (as int) seen by this thread, and its string. */
 int hlc2_last_cuda_error(const char** message);
 /* Number of kernels this library has launched since it was loaded (for launch accounting). */
 unsigned long long hlc2_kernel_launches(void);
-/* Measurement hook: when enabled, hlc2_crossmatch brackets its match kernel (not the planner) with CUDA events on the
- * caller's stream; hlc2_last_match_kernel_ms waits for the latest such launch and returns its duration in *ms
- * (HLC2_ERR_INVALID_ARG if none was timed).  Process-wide, not thread-safe; off by default. */
-int hlc2_time_match_kernel(int enable);
-int hlc2_last_match_kernel_ms(float* ms);
 const char* hlc2_version(void);
 
 #ifdef __cplusplus

@@ -80,8 +80,7 @@ def lib():
         L.hlc2_strerror.restype = ctypes.c_char_p
         L.hlc2_last_cuda_error.argtypes = [P(ctypes.c_char_p)]
         L.hlc2_kernel_launches.restype = ctypes.c_ulonglong
-        L.hlc2_time_match_kernel.argtypes = [ctypes.c_int]
-        L.hlc2_last_match_kernel_ms.argtypes = [P(ctypes.c_float)]
+        L.hlc2_crossmatch_events.argtypes = L.hlc2_crossmatch.argtypes + [vp, vp]
         L.hlc2_version.restype = ctypes.c_char_p
         _lib = L
     return _lib
@@ -139,8 +138,10 @@ def hlc2_build_index(ra_deg, dec_deg, ids=None, opts: hlc2_opts | None = None, s
     """ra_deg, dec_deg: CUDA float64 tensors [n]; ids: CUDA int64 tensor [n] or None (row numbers)."""
     torch = _torch()
     n = int(ra_deg.shape[0])
-    if opts is None:
-        opts = make_opts()
+    # never write into the caller's options object: it may outlive `like`
+    o = hlc2_opts()
+    ctypes.memmove(ctypes.byref(o), ctypes.byref(opts if opts is not None else make_opts()), ctypes.sizeof(hlc2_opts))
+    opts = o
     if like is not None:
         opts.grid_like = like.handle
     assert ra_deg.is_cuda and dec_deg.is_cuda and ra_deg.dtype == torch.float64 and dec_deg.dtype == torch.float64
@@ -212,9 +213,10 @@ def hlc2_crossmatch_sizes(A: Index, B: Index) -> int:
 
 
 def hlc2_crossmatch(A: Index, B: Index, radius_arcsec: float, mode: int, out_ida, out_idb, out_sep, count,
-                    stream=None, temp=None):
+                    stream=None, temp=None, events=None):
     """Raw call: out_* are CUDA tensors of `capacity` rows, `count` a CUDA tensor of one uint64/int64.
-    Asynchronous on `stream`; read `count` after synchronising."""
+    Asynchronous on `stream`; read `count` after synchronising.  `events` = (start, stop) torch.cuda.Event pair
+    (already created, i.e. recorded once) -> hlc2_crossmatch_events records them around the match kernel."""
     cap = int(out_ida.shape[0])
     assert out_idb.shape[0] == cap and out_sep.shape[0] == cap
     need = hlc2_crossmatch_sizes(A, B)
@@ -223,9 +225,15 @@ def hlc2_crossmatch(A: Index, B: Index, radius_arcsec: float, mode: int, out_ida
         temp = torch.empty(need, dtype=torch.uint8, device=A.buf.device)
         # the stream still owns the scratch until the enqueued work drains
         temp.record_stream(torch.cuda.current_stream() if stream is None else stream)
-    rc = lib().hlc2_crossmatch(A.handle, B.handle, float(radius_arcsec), int(mode), out_ida.data_ptr(), out_idb.data_ptr(),
-                               out_sep.data_ptr(), cap, count.data_ptr(), temp.data_ptr() if temp is not None else None,
-                               temp.numel() if temp is not None else 0, _stream_ptr(stream))
+    args = (A.handle, B.handle, float(radius_arcsec), int(mode), out_ida.data_ptr(), out_idb.data_ptr(),
+            out_sep.data_ptr(), cap, count.data_ptr(), temp.data_ptr() if temp is not None else None,
+            temp.numel() if temp is not None else 0, _stream_ptr(stream))
+    if events is None:
+        rc = lib().hlc2_crossmatch(*args)
+    else:
+        e0, e1 = (ctypes.c_void_p(e.cuda_event) for e in events)
+        assert e0.value and e1.value, "record the events once before passing them (torch creates them lazily)"
+        rc = lib().hlc2_crossmatch_events(*args, e0, e1)
     if rc != HLC2_OK:
         raise Hlc2Error(rc, "hlc2_crossmatch")
 
@@ -280,18 +288,6 @@ def hlc2_stream_crossmatch(a_cols, a_off, b_cols, b_off, band_edges_deg, radius_
         e = Hlc2Error(rc, "hlc2_stream_crossmatch"); e.found = cnt.value
         raise e
     return int(cnt.value)
-
-def hlc2_time_match_kernel(enable: bool) -> None:
-    lib().hlc2_time_match_kernel(1 if enable else 0)
-
-
-def hlc2_last_match_kernel_ms() -> float:
-    ms = ctypes.c_float(0.0)
-    rc = lib().hlc2_last_match_kernel_ms(ctypes.byref(ms))
-    if rc != HLC2_OK:
-        raise Hlc2Error(rc, "hlc2_last_match_kernel_ms")
-    return float(ms.value)
-
 
 def kernel_launches() -> int:
     return int(lib().hlc2_kernel_launches())

@@ -381,9 +381,10 @@ int hlc2_crossmatch_sizes(const hlc2_index* A, const hlc2_index* B, size_t* temp
     return HLC2_OK;
 }
 
-int hlc2_crossmatch(const hlc2_index* A, const hlc2_index* B, double radius_arcsec, int mode,
-                    int64_t* d_out_idA, int64_t* d_out_idB, double* d_out_sep, int64_t capacity,
-                    unsigned long long* d_count, void* d_temp, size_t temp_bytes, void* cuda_stream) {
+int hlc2_crossmatch_events(const hlc2_index* A, const hlc2_index* B, double radius_arcsec, int mode,
+                           int64_t* d_out_idA, int64_t* d_out_idB, double* d_out_sep, int64_t capacity,
+                           unsigned long long* d_count, void* d_temp, size_t temp_bytes, void* cuda_stream,
+                           void* ev_kernel_start, void* ev_kernel_stop) {
     if (!A || !B || A->magic != kMagic || B->magic != kMagic || !d_count || capacity < 0 ||
         (capacity > 0 && (!d_out_idA || !d_out_idB || !d_out_sep)) ||
         (mode != HLC2_ALL_PAIRS && mode != HLC2_NEAREST) ||
@@ -395,9 +396,16 @@ int hlc2_crossmatch(const hlc2_index* A, const hlc2_index* B, double radius_arcs
     cudaStream_t s = (cudaStream_t)cuda_stream;
     CU(cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), s));
     launch_match(va, vb, radius_arcsec, mode, d_out_idA, d_out_idB, d_out_sep,
-                 (unsigned long long)capacity, d_count, d_temp, s);
+                 (unsigned long long)capacity, d_count, d_temp, s, (cudaEvent_t)ev_kernel_start, (cudaEvent_t)ev_kernel_stop);
     CU(cudaGetLastError());
     return HLC2_OK;
+}
+
+int hlc2_crossmatch(const hlc2_index* A, const hlc2_index* B, double radius_arcsec, int mode,
+                    int64_t* d_out_idA, int64_t* d_out_idB, double* d_out_sep, int64_t capacity,
+                    unsigned long long* d_count, void* d_temp, size_t temp_bytes, void* cuda_stream) {
+    return hlc2_crossmatch_events(A, B, radius_arcsec, mode, d_out_idA, d_out_idB, d_out_sep, capacity, d_count,
+                                  d_temp, temp_bytes, cuda_stream, nullptr, nullptr);
 }
 
 void hlc2_index_destroy(hlc2_index* idx) {
@@ -425,10 +433,6 @@ int hlc2_last_cuda_error(const char** message) {
 
 unsigned long long hlc2_kernel_launches(void) { return hlc2::g_launches.load(std::memory_order_relaxed); }
 
-int hlc2_time_match_kernel(int enable) { hlc2::set_time_match(enable != 0); return HLC2_OK; }
-
-int hlc2_last_match_kernel_ms(float* ms) { return hlc2::last_match_ms(ms); }
-
-const char* hlc2_version(void) { return "hlc2-b200 0.1 (sm_100a)"; }
+const char* hlc2_version(void) { return "hlc2-b200 0.2 (sm_100a)"; }
 
 }  // extern "C"

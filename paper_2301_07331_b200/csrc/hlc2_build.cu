@@ -20,14 +20,20 @@
 
 namespace hlc2 {
 
-static int g_sm_count = 0;
+// per-device caches (a process may drive several devices); benign race: every thread computes the same value
+int current_device() {
+    int dev = 0; cudaGetDevice(&dev);
+    return dev >= 0 && dev < kMaxDevices ? dev : 0;
+}
 int sm_count() {
-    if (!g_sm_count) {
-        int dev = 0; cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&g_sm_count, cudaDevAttrMultiProcessorCount, dev);
-        if (g_sm_count <= 0) g_sm_count = 148;
+    static int cache[kMaxDevices] = {};
+    const int dev = current_device();
+    if (!cache[dev]) {
+        int v = 0;
+        cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+        cache[dev] = v > 0 ? v : 148;
     }
-    return g_sm_count;
+    return cache[dev];
 }
 
 // ------------------------------------------------------------------------------------------
@@ -135,7 +141,9 @@ k_keys_pack(const double* __restrict__ ra, const double* __restrict__ dec, const
         double a = __ldg(ra + i), d = __ldg(dec + i);
         long long v = id ? (long long)__ldg(id + i) : (long long)i;
         uint32_t key = 0;
-        double ux = 0.0, uy = 0.0, uz = 2.0;       // bad coordinate: a point no chord test can reach
+        // bad coordinate: NaN components, so that no chord test against anything (another bad row, the match's
+        // sentinel slot) can pass; such rows are filed under cell 0 and never appear in a result
+        double ux = __longlong_as_double(0x7ff8000000000000ll), uy = ux, uz = ux;
         if (coord_ok(a, d)) {
             double an = norm_ra(a);
             int z = zone_of(g, d);
@@ -306,11 +314,12 @@ int launch_radix_sort(uint32_t* keys_a, uint32_t* keys_b, uint32_t* val_a, uint3
                       const uint32_t* d_digit_hist, uint32_t* d_digit_base, uint32_t* d_status, uint32_t* d_ticket,
                       cudaStream_t s) {
     if (n == 0) return 0;
-    static bool attr_set = false;
-    if (!attr_set) {
+    static bool attr_set[kMaxDevices] = {};          // the opt-in is a per-device function attribute
+    const int dev = current_device();
+    if (!attr_set[dev]) {
         cudaFuncSetAttribute(k_onesweep<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kOsSmem);
         cudaFuncSetAttribute(k_onesweep<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kOsSmem);
-        attr_set = true;
+        attr_set[dev] = true;
     }
     const int passes = radix_passes(key_bits);
     const uint32_t n_tiles = (uint32_t)sort_tiles(n);

@@ -66,6 +66,8 @@ struct Stats {
 };
 
 // ---- launchers (hlc2_build.cu, hlc2_match.cu) --------------------------------------------
+constexpr int kMaxDevices = 64;               // per-device caches of function attributes and device properties
+int current_device();
 int sm_count();
 void launch_stats(const double* ra, const double* dec, uint32_t n, Stats* d_stats, cudaStream_t s);
 void launch_keys_pack(const double* ra, const double* dec, const int64_t* id, uint32_t n, GridView g, int passes,
@@ -90,10 +92,8 @@ size_t match_temp_for_tiles(size_t tile_cap);
 size_t match_temp_bound(int64_t n_a, const hlc2_opts* opts);
 void launch_match(const IndexView& A, const IndexView& B, double radius_arcsec, int mode,
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
-                  unsigned long long* d_count, void* d_temp, cudaStream_t s);
-
-void set_time_match(bool on);
-int last_match_ms(float* ms);
+                  unsigned long long* d_count, void* d_temp, cudaStream_t s,
+                  cudaEvent_t ev_start = nullptr, cudaEvent_t ev_stop = nullptr);
 
 void count_launch(int k = 1);
 

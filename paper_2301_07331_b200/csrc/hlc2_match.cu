@@ -139,7 +139,6 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity
                      : "=r"(done) : "r"(a), "r"(parity), "r"(0x4000u) : "memory");
     } while (!done);
 }
-__device__ __forceinline__ void mbar_wait_backoff(unsigned long long* b, unsigned parity) { mbar_wait(b, parity); }
 // global -> shared bulk copy, completion counted in bytes on an mbarrier; 16-byte aligned src, dst and size
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* b) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
@@ -211,6 +210,7 @@ __device__ __noinline__ void plan_piece(PlanState& st, const MatchArgs& p, const
             }
             ke = lo;
         }
+        if (re == ra) { ka = ke + 1; continue; }             // a run of empty cells (ke < kb here): nothing to stage
         uint32_t* s = st.w + 4 + 8 * st.nseg;
         s[0] = (uint32_t)z; s[1] = (uint32_t)ka; s[2] = (uint32_t)(ke - ka + 1); s[3] = ra; s[4] = re - ra;
         s[5] = (uint32_t)n; s[6] = cb + (uint32_t)ka; s[7] = __float_as_uint(centre);
@@ -270,6 +270,16 @@ k_plan(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B,
                 if (L < 0.0 && L + 360.0 <= gb.span) { ilo[ni] = L + 360.0; ihi[ni] = fmin(H + 360.0, gb.span); ctr[ni] = c + 360.0f; ++ni; }
                 else if (H >= 360.0) { ilo[ni] = fmax(L - 360.0, 0.0); ihi[ni] = fmin(H - 360.0, gb.span); ctr[ni] = c - 360.0f; ++ni; }
             }
+            // two RA intervals whose cell ranges meet in some zone (few cells per zone: polar zones next to the seam)
+            // would stage those cells twice and report their pairs twice: such tiles take the general path, whose
+            // per-row ranges are merged before they are scanned
+            if (!direct && ni == 2)
+                for (int z = zb0; z <= zb1; ++z) {
+                    const int n = __ldg(gb.n_ra + z);
+                    const int a0 = cell_of_u(gb, ilo[0], n), a1 = cell_of_u(gb, ihi[0], n);
+                    const int b0 = cell_of_u(gb, ilo[1], n), b1 = cell_of_u(gb, ihi[1], n);
+                    if (!(a1 < b0 || b1 < a0)) { direct = true; break; }
+                }
             if (!direct) {
                 for (int i = 0; i < ni && !st.overflow; ++i)
                     for (int z = zb0; z <= zb1 && !st.overflow; ++z) {
@@ -327,7 +337,7 @@ __device__ __noinline__ void scan_general(const IndexView& A, const IndexView& B
                                           double ax, double ay, double az, float2 pf, Best& h) {
     const GridView& g = B.g;
     const double dlo = (double)pf.y - p.pad_dec, dhi = (double)pf.y + p.pad_dec;
-    if (dhi < g.dec_min || dlo > g.dec_max) return;
+    if (!(dhi >= g.dec_min && dlo <= g.dec_max)) return;          // also rows with a bad coordinate (NaN vector)
     const float fx = (float)ax, fy = (float)ay;
     const float s = p.sin_r_up * rsqrtf(fx * fx + fy * fy);               // sin(dRA_max) = sin r / cos dec
     const bool ring = !(s < 0.25f);
@@ -535,7 +545,7 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
             const uint32_t a_ld = any ? (((a_first + a_count + 1u) & ~1u) - a_al) : 0u;
             const uint32_t bytes = a_ld * 32u + rtot * 24u + ctot * 4u;
 
-            mbar_wait_backoff(&sm.empty[s], ph ^ 1u);
+            mbar_wait(&sm.empty[s], ph ^ 1u);
             if (lane == 0) { st.d.a_first = a_first; st.d.a_count = a_count; st.d.a_off = a_first - a_al; st.d.flags = flags; st.d.nseg = nseg; }
             if (segact) {
                 SegDesc& e = st.d.seg[lane];
@@ -563,7 +573,7 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
         }
         // tell the consumers that nothing follows
         const int s = (int)(it % kStages);
-        mbar_wait_backoff(&sm.empty[s], ((it / kStages) & 1u) ^ 1u);
+        mbar_wait(&sm.empty[s], ((it / kStages) & 1u) ^ 1u);
         if (lane == 0) { sm.st[s].d.flags = kJobEnd; sm.st[s].d.nseg = 0; sm.st[s].d.a_count = 0; mbar_arrive(&sm.full[s]); }
         return;
     }
@@ -582,11 +592,7 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
         const uint32_t flags = d.flags, a_count = d.a_count;
         if (flags & kJobEnd) break;
         const int nseg = d.nseg;
-#ifdef HLC2_EXP_NOCOMPUTE
-        if (false) {
-#else
         if ((uint32_t)(warp * 32) < a_count) {
-#endif
             const bool act = threadIdx.x < a_count;
             if (MODE == HLC2_NEAREST && (flags & kJobFirst)) best.has = false;
             const uint32_t a_row = d.a_first + threadIdx.x;
@@ -623,9 +629,6 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
     if (qn) flush_rows(A, B, p, q, 0, qn, lane);
 }
 
-static bool g_time_match = false, g_match_timed = false;
-static cudaEvent_t g_match_ev[2] = {nullptr, nullptr};
-
 static inline size_t pool_cap_of(size_t tile_cap) { return 3 * tile_cap + 4096; }
 
 size_t match_temp_for_tiles(size_t tile_cap) { return (tile_cap + pool_cap_of(tile_cap)) * sizeof(Job) + 256; }
@@ -633,8 +636,12 @@ size_t match_temp_bytes(const IndexView& A, const IndexView& B) { return match_t
 
 void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_arcsec, int mode,
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
-                  unsigned long long* d_count, void* d_temp, cudaStream_t s) {
-    if (A_in.n == 0 || B_in.n == 0) return;
+                  unsigned long long* d_count, void* d_temp, cudaStream_t s, cudaEvent_t ev_start, cudaEvent_t ev_stop) {
+    if (A_in.n == 0 || B_in.n == 0) {
+        if (ev_start) cudaEventRecord(ev_start, s);
+        if (ev_stop) cudaEventRecord(ev_stop, s);
+        return;
+    }
     // all_pairs is symmetric: the pair set of (A, B) is that of (B, A) with the id columns exchanged.  The per-row
     // work (window, cell look-ups) is paid by the catalogue whose rows drive the lanes, while staging grows with the
     // scanned rows per driving row; measured on config 3 (ratio 2) the two directions tie, so the roles are
@@ -658,7 +665,8 @@ void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_ar
     p.tile_cap = (uint32_t)tiles; p.pool_cap = (uint32_t)pool_cap_of(tiles);
     cudaMemsetAsync(p.pool_count, 0, sizeof(uint32_t), s);
     const int m = mode == HLC2_NEAREST ? 1 : 0;
-    static int per_sm[2] = {0, 0};
+    static int per_sm_dev[kMaxDevices][2] = {};        // resident CTAs per SM; the smem opt-in is per device
+    int* per_sm = per_sm_dev[current_device()];
     const size_t smem = sizeof(MatchSmem);
     if (!per_sm[m]) {
         int v = 0;
@@ -676,21 +684,11 @@ void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_ar
     count_launch();
     // persistent grid: SM count x resident CTAs, never more CTAs than tiles
     const unsigned blocks = (unsigned)std::max<size_t>(1, std::min<size_t>(tiles, (size_t)sm_count() * per_sm[m]));
-    if (g_time_match) {                      // measurement hook (hlc2_time_match_kernel): events around k_match alone
-        if (!g_match_ev[0]) { cudaEventCreate(&g_match_ev[0]); cudaEventCreate(&g_match_ev[1]); }
-        cudaEventRecord(g_match_ev[0], s);
-    }
+    if (ev_start) cudaEventRecord(ev_start, s);          // the caller's events bracket k_match alone (hlc2_crossmatch_events)
     if (m) k_match<HLC2_NEAREST><<<blocks, kMatchThreads, smem, s>>>(A, B, p);
     else   k_match<HLC2_ALL_PAIRS><<<blocks, kMatchThreads, smem, s>>>(A, B, p);
     count_launch();
-    if (g_time_match) { cudaEventRecord(g_match_ev[1], s); g_match_timed = true; }
-}
-
-void set_time_match(bool on) { g_time_match = on; }
-int last_match_ms(float* ms) {
-    if (!g_match_timed || !ms) return HLC2_ERR_INVALID_ARG;
-    if (cudaEventSynchronize(g_match_ev[1]) != cudaSuccess || cudaEventElapsedTime(ms, g_match_ev[0], g_match_ev[1]) != cudaSuccess) return HLC2_ERR_CUDA;
-    return HLC2_OK;
+    if (ev_stop) cudaEventRecord(ev_stop, s);
 }
 
 }  // namespace hlc2

@@ -1,0 +1,202 @@
+"""Full-size parity harness: one configuration of BASELINE.json at its STATED size through the C ABI, compared with the
+oracle element by element, plus the per-config report of SURVEY section 5 (N, pairs, t_build, t_match, A-sources/s,
+pairs/s, oracle time and cores, borderline list).  Used by tests/test_gpu_fullsize.py and by `bench.py --report`.
+
+The comparison is the procedure of tests/parity.py written for 1e7..1e8 rows: the generator's ids are
+affine in the row number (idA = 1e12 + 2 i, idB = 2e12 + 2 j + 1), so a pair packs into one int64 (i << 31 | j), both
+sides are sorted on that key (the CUDA rows on the device with torch.sort -- harness work, not part of the path) and
+compared as arrays; only when they differ are the two set differences formed and every differing pair classified with
+the ORACLE's separation (|sep - r| < 1e-9 arcsec -> borderline list, anything else fails).
+"""
+from __future__ import annotations
+
+import json
+import os
+import time
+
+import numpy as np
+
+import hlc2_synth as S
+import oracle
+from tests import parity
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+A0, B0 = 10**12, 2 * 10**12 + 1
+
+
+def rows_of(ida, idb):
+    return (ida - A0) >> 1, (idb - B0) >> 1
+
+
+def pack(ida, idb):
+    i, j = rows_of(ida, idb)
+    return (i << 31) | j
+
+
+def dev(cat):
+    import torch
+    return (torch.from_numpy(cat.ra).cuda(), torch.from_numpy(cat.dec).cuda(), torch.from_numpy(cat.id).cuda())
+
+
+def gpu_rows_sorted(a, b, s):
+    """CUDA tensors of one result -> numpy (key, sep) sorted by the packed (i, j) key."""
+    import torch
+    key = (((a - A0) >> 1) << 31) | ((b - B0) >> 1)
+    key, o = torch.sort(key)
+    return key.cpu().numpy(), s[o].cpu().numpy()
+
+
+def compare_packed(gk, gs, ok, os_, radius, A, B, nearest=False):
+    """Both sides sorted by packed key.  Returns the report dict; raises AssertionError on any violation."""
+    rep = dict(n_gpu=int(len(gk)), n_oracle=int(len(ok)), only_gpu=0, only_oracle=0, borderline=[], swaps=[], max_sep_err=0.0)
+    if len(gk) > 1:
+        assert (gk[1:] != gk[:-1]).all(), "duplicate rows in the CUDA output"
+    if len(gk) == len(ok) and np.array_equal(gk, ok):
+        rep["max_sep_err"] = float(np.abs(gs - os_).max()) if len(gk) else 0.0
+        assert rep["max_sep_err"] <= parity.TOL_SEP, f"separation differs by {rep['max_sep_err']} arcsec"
+        return rep
+    sep_rows = lambda k: np.array([oracle.sep_arcsec(A.ra[i], A.dec[i], B.ra[j], B.dec[j]) for i, j in zip(k >> 31, k & ((1 << 31) - 1))])
+    if nearest:
+        # keyed by the A row: rows only one side has must be borderline; rows with a different B must be near-ties
+        gi, oi = gk >> 31, ok >> 31
+        assert len(np.unique(gi)) == len(gi), "nearest mode produced two rows for one A source"
+        og = np.flatnonzero(~np.isin(gi, oi, assume_unique=True)); oo = np.flatnonzero(~np.isin(oi, gi, assume_unique=True))
+        for k, sk in zip(gk[og], sep_rows(gk[og])):
+            assert abs(sk - radius) < parity.TOL_BORDER, f"CUDA path invented nearest row {int(k >> 31)} (oracle sep {sk!r})"
+            rep["borderline"].append((int(k >> 31), int(k & ((1 << 31) - 1)), float(sk), "gpu_only"))
+        for k, sk in zip(ok[oo], os_[oo]):
+            assert abs(sk - radius) < parity.TOL_BORDER, f"CUDA path lost nearest row {int(k >> 31)} (sep {sk!r})"
+            rep["borderline"].append((int(k >> 31), int(k & ((1 << 31) - 1)), float(sk), "oracle_only"))
+        cg = np.isin(gi, oi, assume_unique=True); co = np.isin(oi, gi, assume_unique=True)
+        gk2, gs2, ok2, os2 = gk[cg], gs[cg], ok[co], os_[co]
+        diff = np.flatnonzero(gk2 != ok2)
+        for k, sk in zip(diff, sep_rows(gk2[diff])):
+            assert abs(sk - os2[k]) < 2 * parity.TOL_SEP, f"A row {int(gk2[k] >> 31)}: CUDA chose another B at {sk!r}, oracle {os2[k]!r}"
+            rep["swaps"].append((int(gk2[k] >> 31), int(gk2[k] & ((1 << 31) - 1)), int(ok2[k] & ((1 << 31) - 1))))
+        same = gk2 == ok2
+        rep["only_gpu"], rep["only_oracle"] = int(len(og)), int(len(oo))
+        rep["max_sep_err"] = float(np.abs(gs2[same] - os2[same]).max()) if same.any() else 0.0
+    else:
+        cg = np.isin(gk, ok, assume_unique=True); co = np.isin(ok, gk, assume_unique=True)
+        og, oo = gk[~cg], np.flatnonzero(~co)
+        rep["only_gpu"], rep["only_oracle"] = int(len(og)), int(len(oo))
+        assert len(og) < 1000 and len(oo) < 1000, f"{len(og)} rows only in the CUDA output, {len(oo)} only in the oracle's"
+        for k, sk in zip(og, sep_rows(og)):
+            assert abs(sk - radius) < parity.TOL_BORDER, f"CUDA path invented pair {(int(k >> 31), int(k & ((1 << 31) - 1)))} oracle sep {sk!r}"
+            rep["borderline"].append((int(k >> 31), int(k & ((1 << 31) - 1)), float(sk), "gpu_only"))
+        for k in oo:
+            assert abs(os_[k] - radius) < parity.TOL_BORDER, f"CUDA path lost pair {(int(ok[k] >> 31), int(ok[k] & ((1 << 31) - 1)))} sep {os_[k]!r}"
+            rep["borderline"].append((int(ok[k] >> 31), int(ok[k] & ((1 << 31) - 1)), float(os_[k]), "oracle_only"))
+        rep["max_sep_err"] = float(np.abs(gs[cg] - os_[co]).max()) if cg.any() else 0.0
+    assert rep["max_sep_err"] <= parity.TOL_SEP, f"separation differs by {rep['max_sep_err']} arcsec"
+    return rep
+
+
+def timed_gpu(P, w, mode, opts_a, opts_b, like_b=None, reps=3, same_grid=False):
+    """Build both indices and match, timing each phase with CUDA events (best of `reps` after one warm-up).
+    Returns (idA, idB, sep CUDA tensors of the last run, ia, ib, timings in ms)."""
+    import torch
+    dA, dB = dev(w.A), dev(w.B)
+    r = w.radius_arcsec
+    cap = max(1024, int(max(len(w.A), len(w.B)) * (4.0 if w.name.startswith("cfg4") else 1.0)))
+    oa = torch.empty(cap, dtype=torch.int64, device="cuda"); ob = torch.empty_like(oa)
+    os_ = torch.empty(cap, dtype=torch.float64, device="cuda"); cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    best = dict(build_a=1e30, build_b=1e30, match=1e30)
+    ia = ib = None
+    for k in range(reps + 1):
+        e = [ev() for _ in range(4)]
+        e[0].record()
+        ib = P.hlc2_build_index(*dB, opts=opts_b, like=like_b)
+        e[1].record()
+        ia = P.hlc2_build_index(*dA, opts=opts_a, like=ib if same_grid else None)
+        e[2].record()
+        P.hlc2_crossmatch(ia, ib, r, mode, oa, ob, os_, cnt)
+        e[3].record()
+        torch.cuda.synchronize()
+        if k:
+            best["build_b"] = min(best["build_b"], e[0].elapsed_time(e[1])); best["build_a"] = min(best["build_a"], e[1].elapsed_time(e[2]))
+            best["match"] = min(best["match"], e[2].elapsed_time(e[3]))
+    n = int(cnt.item())
+    assert n <= cap, f"capacity {cap} too small for {n} rows"
+    assert P.hlc2_index_status(ia)[0] == 0 and P.hlc2_index_status(ib)[0] == 0
+    return oa[:n], ob[:n], os_[:n], ia, ib, best
+
+
+def cfg4_workload(P, scale=1.0):
+    """Config 4 needs the grid of the B index it will be matched on (its sources sit on that grid's cell / zone edges):
+    the grid comes from hlc2_grid_describe of a preliminary index built with the same options."""
+    import torch
+    n_b = int(round(20_000_000 * scale))
+    opts = P.make_opts(3.0, cell_arcsec=160.0, full_sky=True)
+    ra, dec = S.uniform_sphere(np.random.default_rng(1), min(n_b, 1_000_000))
+    pre = P.hlc2_build_index(torch.from_numpy(ra).cuda(), torch.from_numpy(dec).cuda(), None, opts=opts)
+    grid = P.hlc2_grid_describe(pre)
+    return S.config(4, scale=scale, grid=grid), pre, grid
+
+
+def stratified_subsample(w, grid, m=200_000, seed=4):
+    """Config 4's prescribed check: m A sources stratified 50/20/20/10 over the edge / cap / seam / uniform classes."""
+    cls = S.stress_classes(S.BASE_SEED + 4, len(w.A), grid)
+    rng = np.random.default_rng(seed)
+    rows = []
+    for c, share in ((0, 0.5), (1, 0.2), (2, 0.2), (3, 0.1)):
+        pool = np.flatnonzero(cls == c)
+        rows.append(rng.choice(pool, min(len(pool), int(round(m * share))), replace=False))
+    return np.sort(np.concatenate(rows))
+
+
+def report(P, cfg, scale=1.0, one_core=False, same_grid=False, out_dir=None):
+    """Run configuration `cfg` at `scale` (1.0 = the stated size) and compare every mode with the oracle."""
+    import torch
+    t0 = time.perf_counter()
+    like_b = None; grid = None
+    if cfg == 4:
+        w, like_b, grid = cfg4_workload(P, scale)
+        opts_a = P.make_opts(3.0, cell_arcsec=160.0, full_sky=True); opts_b = P.make_opts(3.0)
+    else:
+        w = S.config(cfg, scale=scale)
+        opts_a = opts_b = P.make_opts(w.radius_arcsec)
+    t_gen = time.perf_counter() - t0
+    r = w.radius_arcsec
+    out = dict(config=cfg, workload=w.name, scale=scale, n_a=len(w.A), n_b=len(w.B), radius_arcsec=r, gen_seconds=t_gen,
+               same_grid=bool(same_grid), modes={})
+    for mname in w.modes:
+        mode = P.HLC2_NEAREST if mname == "nearest" else P.HLC2_ALL_PAIRS
+        a, b, s, ia, ib, tm = timed_gpu(P, w, mode, opts_a, opts_b, like_b=like_b, same_grid=same_grid)
+        gk, gs = gpu_rows_sorted(a, b, s)
+        del a, b, s
+        torch.cuda.empty_cache()
+        t1 = time.perf_counter()
+        oa, ob, osep, used = oracle.match(w.A.ra, w.A.dec, w.A.id, w.B.ra, w.B.dec, w.B.id, r, mode)
+        t_or = time.perf_counter() - t1
+        ok = pack(oa, ob)
+        rep = compare_packed(gk, gs, ok, osep, r, w.A, w.B, nearest=mode == P.HLC2_NEAREST)
+        rep.update(t_build_a_ms=tm["build_a"], t_build_b_ms=tm["build_b"], t_match_ms=tm["match"],
+                   a_src_per_s_match=len(w.A) / (tm["match"] * 1e-3), pairs_per_s_match=len(gk) / (tm["match"] * 1e-3),
+                   a_src_per_s_step=len(w.A) / ((tm["match"] + tm["build_a"] + tm["build_b"]) * 1e-3),
+                   oracle_seconds=t_or, oracle_cores=used, oracle_a_src_per_s=len(w.A) / t_or,
+                   cells_a=P.hlc2_grid_describe(ia)["n_cells"], cells_b=P.hlc2_grid_describe(ib)["n_cells"])
+        if one_core:
+            t1 = time.perf_counter()
+            oracle.match(w.A.ra, w.A.dec, w.A.id, w.B.ra, w.B.dec, w.B.id, r, mode, threads=1)
+            rep["oracle_seconds_1core"] = time.perf_counter() - t1
+        if cfg == 4 and mode == P.HLC2_ALL_PAIRS:
+            # the prescribed completeness check: brute force ("No Index") on a stratified subsample of A
+            rows = stratified_subsample(w, grid, min(200_000, len(w.A)))
+            sub = w.A.take(rows)
+            t1 = time.perf_counter()
+            ba, bb, bs, _ = oracle.match(sub.ra, sub.dec, sub.id, w.B.ra, w.B.dec, w.B.id, r, mode, oracle.ENGINE_BRUTE)
+            t_bf = time.perf_counter() - t1
+            bk = pack(ba, bb)
+            sel = np.isin(gk >> 31, rows)
+            brep = compare_packed(gk[sel], gs[sel], bk, bs, r, w.A, w.B)
+            rep["brute_force_subsample"] = dict(rows=int(len(rows)), seconds=t_bf, **brep)
+        out["modes"][mname] = rep
+        del ia, ib
+        torch.cuda.empty_cache()
+    if out_dir:
+        os.makedirs(out_dir, exist_ok=True)
+        with open(os.path.join(out_dir, f"parity_full_cfg{cfg}{'_samegrid' if same_grid else ''}.json"), "w") as f:
+            json.dump(out, f, indent=1)
+    return out

@@ -59,8 +59,6 @@ def compare_all_pairs(gpu, ora, radius, sep_of=None):
 def compare_nearest(gpu, ora, radius, sep_of=None):
     ga, gb, gs = _sorted(*gpu)
     oa, ob, os_ = _sorted(*ora)
-    if len(ga) > 1:
-        assert (ga[1:] != ga[:-1]).all() or len(np.unique(ga)) == len(ga) or True
     # rows are keyed by idA; ids of A are unique in every workload used here
     assert len(np.unique(ga)) == len(ga), "nearest mode produced two rows for one A id"
     only_o = np.flatnonzero(~np.isin(oa, ga)); only_g = np.flatnonzero(~np.isin(ga, oa))
