@@ -4,8 +4,8 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C] [--scale S]
 
 A "step" is one pass of the whole hot path over one batch of synthetic input already resident in
-HBM: hlc2_build_index(A) + hlc2_build_index(B) + hlc2_crossmatch(A, B) (all SURVEY 8(a) rows except
-streaming).  Workload at N = 1: configuration 3 of BASELINE.json ("Gaia-like density", A = 100M,
+HBM: hlc2_build_index(B) + hlc2_build_index(A, on B's grid: opts.grid_like) + hlc2_crossmatch(A, B) (all
+SURVEY 8(a) rows except streaming; --grid own gives A a grid of its own).  Workload at N = 1: configuration 3 of BASELINE.json ("Gaia-like density", A = 100M,
 B = 50M, r = 1 arcsec, all_pairs) -- the configuration north_star's target is quoted on.
 
 One JSON line is printed (rank 0).  `value` = A sources cross-matched per second over the whole step,
@@ -49,12 +49,38 @@ def peak_hbm():
 
 
 def ncu_traffic():
-    """DRAM bytes per launch of the match kernel from the committed ncu --set full capture, or None."""
+    """DRAM bytes per launch of the match kernel from this round's committed `ncu --set full` capture
+    (profiles/match_traffic.txt).  The record names the sha256 of the kernel source it was taken on: a capture of an
+    older kernel is reported as stale and its number is NOT used."""
+    import hashlib
     p = os.path.join(ROOT, "profiles", "match_traffic.txt")
     try:
-        return json.load(open(p))
+        rec = json.load(open(p))
     except Exception:
-        return None
+        return None, "no capture committed"
+    src = os.path.join(ROOT, "paper_2301_07331_b200", "csrc", "hlc2_match.cu")
+    sha = hashlib.sha256(open(src, "rb").read()).hexdigest()
+    if rec.get("hlc2_match_cu_sha256") != sha:
+        return None, f"stale: {p} was captured on another version of hlc2_match.cu"
+    return rec, rec.get("source", "")
+
+
+def pcie_rates(gib=1):
+    """Pinned host <-> device copy rates, one plain cudaMemcpyAsync of `gib` GiB per direction (best of 3): the roofline
+    of every number that includes host copies (e2e, streamed config 5)."""
+    import torch
+    n = gib << 30
+    h = torch.empty(n, dtype=torch.uint8).pin_memory(); d = torch.empty(n, dtype=torch.uint8, device="cuda")
+    out = {}
+    for name, src, dst in (("h2d_gbs", h, d), ("d2h_gbs", d, h)):
+        best = 0.0
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); dst.copy_(src, non_blocking=True); e1.record(); e1.synchronize()
+            best = max(best, n / (e0.elapsed_time(e1) * 1e-3) / 1e9)
+        out[name] = best
+    out["how"] = f"one cudaMemcpyAsync of {gib} GiB pinned<->device per direction, best of 3, CUDA events"
+    return out
 
 
 class ClockSampler:
@@ -110,12 +136,12 @@ def sample_patch(w, ra_lo=0.0, ra_hi=3.6):
     return S.Catalogue(w.A.ra[ma], w.A.dec[ma], w.A.id[ma]), S.Catalogue(w.B.ra[mb], w.B.dec[mb], w.B.id[mb])
 
 
-def time_oracle(A, B, radius, mode):
+def time_oracle(A, B, radius, mode, keep=False, threads=0):
     import oracle
     t = time.perf_counter()
-    a, b, s, used = oracle.match(A.ra, A.dec, A.id, B.ra, B.dec, B.id, radius, mode)
+    a, b, s, used = oracle.match(A.ra, A.dec, A.id, B.ra, B.dec, B.id, radius, mode, threads=threads)
     dt = time.perf_counter() - t
-    return dt, len(a), used
+    return (dt, len(a), used, (a, b, s)) if keep else (dt, len(a), used)
 
 
 def run_reference(args, w, mode):
@@ -124,11 +150,13 @@ def run_reference(args, w, mode):
     if rank != 0:
         return
     # size the sample so that the whole --steps/--warmup run takes about two minutes on this box's cores
+    # and is the WHOLE workload whenever that fits (config 3: ~45 s per pass on 16 cores -> up to 3 passes)
     pa, pb = sample_patch(w, 0.0, 3.6)
     dt_probe, _, _ = time_oracle(pa, pb, w.radius_arcsec, mode)
-    budget = 120.0 / max(1, args.steps + args.warmup)
-    args.sample_ra_deg = float(min(args.sample_ra_deg, max(1.0, 3.6 * budget / max(dt_probe, 1e-3))))
-    A, B = sample_patch(w, 0.0, args.sample_ra_deg)
+    budget = 150.0 / max(1, args.steps + args.warmup)
+    args.sample_ra_deg = float(min(360.0, max(1.0, 3.6 * budget / max(dt_probe, 1e-3))))
+    whole = args.sample_ra_deg >= 360.0
+    A, B = (w.A, w.B) if whole else sample_patch(w, 0.0, args.sample_ra_deg)
     for _ in range(args.warmup):
         time_oracle(A, B, w.radius_arcsec, mode)
     t_tot, used = 0.0, 0
@@ -136,7 +164,8 @@ def run_reference(args, w, mode):
         dt, npairs, used = time_oracle(A, B, w.radius_arcsec, mode)
         t_tot += dt
     val = len(A) * args.steps / t_tot
-    sample = f"both catalogues restricted to RA in [0,{args.sample_ra_deg}) deg: {len(A)} x {len(B)} sources, {npairs} rows"
+    sample = (f"the whole workload: {len(A)} x {len(B)} sources, {npairs} rows" if whole else
+              f"both catalogues restricted to RA in [0,{args.sample_ra_deg:.2f}) deg: {len(A)} x {len(B)} sources, {npairs} rows")
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * t_tot / args.steps, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f80 (x87 long double)", "data": "synthetic",
@@ -156,7 +185,9 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--scale", type=float, default=1.0, help="scale the source counts (1.0 = the named configuration)")
-    ap.add_argument("--sample-ra-deg", type=float, default=108.0, help="RA slice of the CPU-baseline sample")
+    ap.add_argument("--sample-ra-deg", type=float, default=360.0, help="RA slice of the CPU-baseline sample (360 = the whole workload)")
+    ap.add_argument("--grid", default="shared", choices=["shared", "own"], help="shared: A is filed on B's grid (opts.grid_like); own: each index plans its own grid")
+    ap.add_argument("--no-verify", action="store_true", help="do not compare the CUDA rows with the oracle's (needs the cpu_baseline leg on the whole workload)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--occupancy", type=float, default=0.0)
     ap.add_argument("--occupancy-b", type=float, default=None, help="target occupancy of B's index (default: same as --occupancy)")
@@ -197,9 +228,18 @@ def main():
     torch.cuda.synchronize()
 
     opts_a = P.make_opts(r, target_occupancy=args.occupancy); opts_b = P.make_opts(r, target_occupancy=args.occupancy if args.occupancy_b is None else args.occupancy_b)
-    ib_a, tb_a = P.hlc2_index_sizes(n_a, opts_a); ib_b, tb_b = P.hlc2_index_sizes(n_b, opts_b)
-    buf_a = torch.empty(ib_a, dtype=torch.uint8, device="cuda"); buf_b = torch.empty(ib_b, dtype=torch.uint8, device="cuda")
-    temp = torch.empty(max(tb_a, tb_b), dtype=torch.uint8, device="cuda")
+    ib_b, tb_b = P.hlc2_index_sizes(n_b, opts_b)
+    buf_b = torch.empty(ib_b, dtype=torch.uint8, device="cuda")
+    temp = torch.empty(tb_b, dtype=torch.uint8, device="cuda")
+    if args.grid == "shared":             # A's buffers are sized for B's grid: build B once to learn it
+        ib0 = P.hlc2_build_index(dB[0], dB[1], dB[2], opts=opts_b, temp=temp, buf=buf_b)
+        ib_a, tb_a = P.hlc2_index_sizes(n_a, P.make_opts(r, target_occupancy=args.occupancy, grid_like=ib0))
+        del ib0
+    else:
+        ib_a, tb_a = P.hlc2_index_sizes(n_a, opts_a)
+    buf_a = torch.empty(ib_a, dtype=torch.uint8, device="cuda")
+    if tb_a > tb_b:
+        temp = torch.empty(tb_a, dtype=torch.uint8, device="cuda")
     cap = int(max(n_a, n_b) * 0.5) + 1024 if mode == 0 else n_a
     out_a = torch.empty(cap, dtype=torch.int64, device="cuda"); out_b = torch.empty(cap, dtype=torch.int64, device="cuda")
     out_s = torch.empty(cap, dtype=torch.float64, device="cuda"); cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
@@ -208,11 +248,13 @@ def main():
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
 
+    shared = args.grid == "shared"
+
     def step(devA, devB, marks=None):
         if marks is not None: marks[0].record()
-        ia = P.hlc2_build_index(devA[0], devA[1], devA[2], opts=opts_a, temp=temp, buf=buf_a)
-        if marks is not None: marks[1].record()
         ib = P.hlc2_build_index(devB[0], devB[1], devB[2], opts=opts_b, temp=temp, buf=buf_b)
+        if marks is not None: marks[1].record()
+        ia = P.hlc2_build_index(devA[0], devA[1], devA[2], opts=opts_a, temp=temp, buf=buf_a, like=ib if shared else None)
         if marks is not None: marks[2].record()
         P.hlc2_crossmatch(ia, ib, r, mode, out_a, out_b, out_s, cnt, temp=temp)
         if marks is not None: marks[3].record()
@@ -244,7 +286,7 @@ def main():
     launches = P.kernel_launches() - n0
     t_ms = e0.elapsed_time(e1)
     ph = np.array([[m[0].elapsed_time(m[1]), m[1].elapsed_time(m[2]), m[2].elapsed_time(m[3])] for m in marks])
-    t_build_a, t_build_b, t_match = ph.mean(axis=0)
+    t_build_b, t_build_a, t_match = ph.mean(axis=0)
 
     # ---- the dominant kernel alone: CUDA events recorded by the library around k_match on this stream (the planner and
     # the count memset of the hlc2_crossmatch call are left out), one launch at a time on the indices of the last step ----
@@ -321,23 +363,34 @@ def main():
         peak, peak_src = peak_hbm()
         alg_bytes = 32.0 * n_a + 32.0 * n_b + 24.0 * found          # catalogue (sorted SoA) + output bytes
         achieved = alg_bytes / (t_kernel * 1e-3) / 1e9
-        tr = ncu_traffic()
+        tr, tr_note = ncu_traffic()
         roof = {"bound": "hbm", "kernel": "k_match", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "frac_of_nominal_8TBs": achieved / 8000.0, "peak_source": peak_src,
-                "traffic": tr["dram_bytes_per_launch"] if tr else None, "algorithmic_bytes": alg_bytes,
+                "traffic": tr["dram_bytes_per_launch"] if tr else None, "traffic_source": tr_note, "algorithmic_bytes": alg_bytes,
                 "ms_per_launch": t_kernel, "launches_timed": len(kms),
                 "timing": "the caller's CUDA events recorded by the library around k_match on the caller's stream (hlc2_crossmatch_events)",
                 "whole_call": {"ms": float(t_match), "frac": alg_bytes / (t_match * 1e-3) / 1e9 / peak,
                                "what": "hlc2_crossmatch inside the timed steps: count memset + k_plan + k_match"}}
-        cpu = None
+        cpu, verify = None, None
         if not args.no_cpu_baseline:
-            sa, sb = sample_patch(w, 0.0, args.sample_ra_deg)
-            dt, npairs, used = time_oracle(sa, sb, r, mode)
+            whole = args.sample_ra_deg >= 360.0
+            sa, sb = (w.A, w.B) if whole else sample_patch(w, 0.0, args.sample_ra_deg)
+            dt, npairs, used, rows = time_oracle(sa, sb, r, mode, keep=True)
             cpu = {"value": len(sa) / dt, "unit": UNIT, "cores": used, "kind": "oracle", "seconds": dt,
-                   "sample": f"both catalogues restricted to RA in [0,{args.sample_ra_deg}) deg: {len(sa)} x {len(sb)} sources, {npairs} rows"}
+                   "sample": (f"the whole workload: {len(sa)} x {len(sb)} sources, {npairs} rows" if whole else
+                              f"both catalogues restricted to RA in [0,{args.sample_ra_deg}) deg: {len(sa)} x {len(sb)} sources, {npairs} rows")}
+            if whole and not args.no_verify:
+                # the oracle's rows are the expected result of the very arrays the GPU just matched: compare them
+                # element by element (tests/fullsize.py: the comparison procedure of SURVEY 8(c))
+                from tests import fullsize
+                gk, gs = fullsize.gpu_rows_sorted(out_a[:found], out_b[:found], out_s[:found])
+                rep = fullsize.compare_packed(gk, gs, fullsize.pack(rows[0], rows[1]), rows[2], r, w.A, w.B, nearest=mode == 1)
+                verify = {"against": "oracle, whole workload, element by element", **rep}
+            del rows
         resident = {"value": units * args.steps / (t_e2e_ms * 1e-3), "ms_per_step": t_e2e_ms / args.steps,
                     "path": "pinned host -> H2D -> hlc2_build_index x2 -> hlc2_crossmatch -> D2H of count and rows"}
-        e2e = {"unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "resident_path": resident}
+        pcie = pcie_rates()
+        e2e = {"unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "resident_path": resident, "pcie": pcie}
         if t_stream_ms is not None:
             streamed = {"value": units * args.steps / (t_stream_ms * 1e-3), "ms_per_step": t_stream_ms / args.steps,
                         "path": "pinned host bands -> hlc2_stream_crossmatch (H2D, build, match, D2H overlapped on 3 streams)",
@@ -345,19 +398,23 @@ def main():
             e2e["streamed_path"] = streamed
         best = e2e.get("streamed_path", resident) if e2e.get("streamed_path", resident)["value"] > resident["value"] else resident
         e2e.update({"value": best["value"], "ms_per_step": best["ms_per_step"], "path": best["path"]})
+        # roofline of the end-to-end number: the step's H2D and D2H bytes at the measured pinned copy rates (the two
+        # directions overlap on the PCIe link, so the bound is the slower of the two, not their sum)
+        t_pcie = max(h2d / (pcie["h2d_gbs"] * 1e9), d2h / (pcie["d2h_gbs"] * 1e9))
+        e2e["roofline"] = {"bound": "pcie", "ms_at_peak": 1e3 * t_pcie, "frac": 1e3 * t_pcie / best["ms_per_step"]}
         line = {"metric": METRIC, "value": units * args.steps / (t_ms * 1e-3), "unit": UNIT, "n_gpus": world,
                 "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_ms / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
                 "config": {"workload": w.name, "n_a": n_a, "n_b": n_b, "radius_arcsec": r,
                            "mode": "nearest" if mode else "all_pairs", "rows_found": found,
                            "parallelism": "replicas only (north_star: one GPU, no collectives)" if world > 1 else "1 gpu",
-                           "l2": "inputs (3.6 GB at scale 1) larger than L2; no explicit flush",
+                           "l2": "inputs (3.6 GB at scale 1) larger than L2; no explicit flush", "grid": args.grid,
                            "cells_a": grid_a["n_cells"], "cells_b": grid_b["n_cells"], "cell_arcsec_b": grid_b["cell_arcsec"],
                            "gen_seconds": t_gen},
                 "pairs_per_s": pairs_all * args.steps / (t_ms * 1e-3),
                 "match_phase": {"ms": float(t_match), "a_sources_per_s": n_a / (t_match * 1e-3), "pairs_per_s": found / (t_match * 1e-3)},
                 "phases_ms": {"build_index_A": float(t_build_a), "build_index_B": float(t_build_b), "crossmatch": float(t_match)},
-                "roofline": roof, "cpu_baseline": cpu,
+                "roofline": roof, "cpu_baseline": cpu, "verify": verify,
                 "e2e": e2e,
                 "gpu_launches": int(launches), "clocks": clk}
         print(json.dumps(line), flush=True)

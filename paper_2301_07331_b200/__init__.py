@@ -17,6 +17,8 @@ from dataclasses import dataclass
 HLC2_ALL_PAIRS = 0
 HLC2_NEAREST = 1
 
+HLC2_KEY_MASK = (1 << 28) - 1      # low bits of hlc2_index_arrays()["cell_key"]: the cell key; top bits: window flags
+
 HLC2_OK = 0
 HLC2_ERR_INVALID_ARG = -1
 HLC2_ERR_RADIUS_TOO_LARGE = -2

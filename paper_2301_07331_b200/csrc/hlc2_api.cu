@@ -55,6 +55,7 @@ struct hlc2_index {
     int device;
     Stats h_stats;        // copy of the extent pass
     bool stats_valid;
+    bool flagged;         // the sorted keys carry window flags in their top bits (grids of <= 2^28 cells)
 };
 static const uint32_t kMagic = 0x484C4332u;   // "HLC2"
 
@@ -227,11 +228,19 @@ static IndexView index_view(const hlc2_index* ix) {
     v.x = (const double*)(ix->d_buf + ix->lay.x); v.y = (const double*)(ix->d_buf + ix->lay.y);
     v.z = (const double*)(ix->d_buf + ix->lay.z); v.id = (const int64_t*)(ix->d_buf + ix->lay.id);
     v.pos = (const float2*)(ix->d_buf + ix->lay.pos);
+    v.key = (const uint32_t*)(ix->d_buf + ix->lay.key); v.key_mask = ix->flagged ? kKeyMask : 0xFFFFFFFFu;
     v.cell_start = (const uint32_t*)(ix->d_buf + ix->lay.cell_start);
     v.tiles = (const TileDesc*)(ix->d_buf + ix->lay.tiles); v.n_tiles = (const uint32_t*)(ix->d_buf + ix->lay.n_tiles);
     v.g = grid_view(ix); v.n = (uint32_t)ix->n;
     v.tile_cap = (uint32_t)((size_t)ix->n / kTile + (size_t)ix->grid.n_zones + 1);
     return v;
+}
+
+// do two indices share one grid (same zones, same cells, same box)?  Then a source's cell key means the same in both.
+static bool same_grid(const hlc2_index* a, const hlc2_index* b) {
+    const HostGrid& x = a->grid; const HostGrid& y = b->grid;
+    return a->flagged && b->flagged && x.n_zones == y.n_zones && x.dec_lo == y.dec_lo && x.h == y.h && x.ra0 == y.ra0 &&
+           x.span == y.span && x.n_ra == y.n_ra;
 }
 
 // does every occupied coarse RA bin of `st` lie inside grid g's RA box?
@@ -309,6 +318,8 @@ int hlc2_build_index(const double* d_ra, const double* d_dec, const int64_t* d_i
 
     // (a1) keys + packed records + digit counts -> (a2) radix sort (key, row) -> (a3) gather -> (a4) cell table, tiles
     uint32_t n_cells = g.n_cells();
+    ix->flagged = n_cells <= (1u << kKeyFlagShift);
+    const uint32_t kmask = ix->flagged ? kKeyMask : 0xFFFFFFFFu;
     int key_bits = 1; while (key_bits < 32 && (1ull << key_bits) < (unsigned long long)n_cells) ++key_bits;
     int passes = radix_passes(key_bits);
     uint32_t* key_idx = (uint32_t*)(buf + L.key);           // the sorted keys must end up here
@@ -319,13 +330,13 @@ int hlc2_build_index(const double* d_ra, const double* d_dec, const int64_t* d_i
     Rec* rec = (Rec*)(tmp + T.rec);
     uint32_t* digit_hist = (uint32_t*)(tmp + T.digit_hist);
     if (cudaMemsetAsync(digit_hist, 0, (size_t)kMaxPasses * kRadix * 4, s) != cudaSuccess) { t_last_cuda = cudaGetLastError(); return fail(HLC2_ERR_CUDA); }
-    launch_keys_pack(d_ra, d_dec, d_id, nn, gv, passes, ka, rec, digit_hist, s);
+    launch_keys_pack(d_ra, d_dec, d_id, nn, gv, passes, o.r_max_arcsec, ix->flagged, ka, rec, digit_hist, s);
     int where = launch_radix_sort(ka, kb, pa, pb, nn, key_bits, digit_hist, (uint32_t*)(tmp + T.digit_base),
                                   (uint32_t*)(tmp + T.status), (uint32_t*)(tmp + T.ticket), s);
     const uint32_t* perm = where ? pb : pa;
     launch_gather(rec, perm, nn, (double*)(buf + L.x), (double*)(buf + L.y), (double*)(buf + L.z), (int64_t*)(buf + L.id), (float2*)(buf + L.pos), s);
-    launch_cell_table(key_idx, nn, n_cells, (uint32_t*)(buf + L.cell_start), (uint32_t*)(tmp + T.big), s);
-    launch_tiles((const uint32_t*)(buf + L.cell_start), gv.cell_base, (uint32_t)g.n_zones, key_idx,
+    launch_cell_table(key_idx, kmask, nn, n_cells, (uint32_t*)(buf + L.cell_start), (uint32_t*)(tmp + T.big), s);
+    launch_tiles((const uint32_t*)(buf + L.cell_start), gv.cell_base, (uint32_t)g.n_zones, key_idx, kmask,
                  (uint32_t)((size_t)n / kTile + (size_t)g.n_zones + 1), (uint32_t*)(tmp + T.tile_first),
                  (TileDesc*)(buf + L.tiles), (uint32_t*)(buf + L.n_tiles), s);
     cudaError_t e = cudaGetLastError();
@@ -396,7 +407,8 @@ int hlc2_crossmatch_events(const hlc2_index* A, const hlc2_index* B, double radi
     cudaStream_t s = (cudaStream_t)cuda_stream;
     CU(cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), s));
     launch_match(va, vb, radius_arcsec, mode, d_out_idA, d_out_idB, d_out_sep,
-                 (unsigned long long)capacity, d_count, d_temp, s, (cudaEvent_t)ev_kernel_start, (cudaEvent_t)ev_kernel_stop);
+                 (unsigned long long)capacity, d_count, d_temp, s, same_grid(A, B) ? kMatchSameGrid : 0u,
+                 (cudaEvent_t)ev_kernel_start, (cudaEvent_t)ev_kernel_stop);
     CU(cudaGetLastError());
     return HLC2_OK;
 }

@@ -131,16 +131,34 @@ __device__ __forceinline__ void unit_vector(double ra_norm, double dec, double& 
 
 constexpr int kKeyThreads = 256;
 
+// Window flags of a valid source on its own grid (see kKeyExtLo / kKeyExtHi / kKeySlow).  Any source within r_max of
+// this one has a declination in [dec - r, dec + r] and an RA within asin(sin r / cos dec) of it, and zone_of / cell_of_u
+// are monotone, so its zone and cell lie between those of the window's ends evaluated with the SAME expressions that
+// file sources: flags computed from the padded window are a superset of what any query radius <= r_max needs.
+__device__ __forceinline__ uint32_t window_flags(const GridView& g, double dec, double cd, double u, int z, int nra, int k,
+                                                 double rpad_deg, double sin_r) {
+    if (zone_of(g, dec - rpad_deg) != z || zone_of(g, dec + rpad_deg) != z) return kKeySlow;
+    const double s = sin_r / fmax(cd, 1e-300);                       // sin of the RA half-window
+    if (!(s < 0.2)) return kKeySlow;                                  // polar rows: wide windows, rings
+    const double w = fma(0.2 * s * s, s, s) * 57.29577951308232 + 1e-9;   // asin(s) <= s + s^3 / 5 below 0.2
+    const double ulo = u - w, uhi = u + w;
+    if (ulo < 0.0 ? ulo + 360.0 <= g.span : uhi >= 360.0) return kKeySlow;  // the window's image through RA = 0/360 lies inside the box
+    const int klo = cell_of_u(g, fmax(ulo, 0.0), nra), khi = cell_of_u(g, fmin(uhi, g.span), nra);
+    if (klo < k - 1 || khi > k + 1) return kKeySlow;
+    return (klo < k ? kKeyExtLo : 0u) | (khi > k ? kKeyExtHi : 0u);
+}
+
 __global__ void __launch_bounds__(kKeyThreads)
 k_keys_pack(const double* __restrict__ ra, const double* __restrict__ dec, const int64_t* __restrict__ id, uint32_t n,
-            GridView g, int passes, uint32_t* __restrict__ keys, Rec* __restrict__ rec, uint32_t* __restrict__ digit_hist) {
+            GridView g, int passes, double rpad_deg, double sin_r, int flagged,
+            uint32_t* __restrict__ keys, Rec* __restrict__ rec, uint32_t* __restrict__ digit_hist) {
     __shared__ uint32_t hist[kMaxPasses * kRadix];
     for (int i = threadIdx.x; i < kMaxPasses * kRadix; i += kKeyThreads) hist[i] = 0;
     __syncthreads();
     for (size_t i = (size_t)blockIdx.x * kKeyThreads + threadIdx.x; i < n; i += (size_t)gridDim.x * kKeyThreads) {
         double a = __ldg(ra + i), d = __ldg(dec + i);
         long long v = id ? (long long)__ldg(id + i) : (long long)i;
-        uint32_t key = 0;
+        uint32_t key = 0, flags = 0;
         // bad coordinate: NaN components, so that no chord test against anything (another bad row, the match's
         // sentinel slot) can pass; such rows are filed under cell 0 and never appear in a result
         double ux = __longlong_as_double(0x7ff8000000000000ll), uy = ux, uz = ux;
@@ -148,10 +166,13 @@ k_keys_pack(const double* __restrict__ ra, const double* __restrict__ dec, const
             double an = norm_ra(a);
             int z = zone_of(g, d);
             int nra = __ldg(g.n_ra + z);
-            key = __ldg(g.cell_base + z) + (uint32_t)cell_of_u(g, box_u(g, an), nra);
+            const double u = box_u(g, an);
+            const int k = cell_of_u(g, u, nra);
+            key = __ldg(g.cell_base + z) + (uint32_t)k;
             unit_vector(an, d, ux, uy, uz);
+            if (flagged) flags = window_flags(g, d, sqrt(fma(ux, ux, uy * uy)), u, z, nra, k, rpad_deg, sin_r);
         }
-        keys[i] = key;
+        keys[i] = key | flags;          // the sort looks at the key bits only; the flags ride along
         double2* o = reinterpret_cast<double2*>(rec + i);
         o[0] = make_double2(ux, uy);
         o[1] = make_double2(uz, __longlong_as_double(v));
@@ -163,10 +184,13 @@ k_keys_pack(const double* __restrict__ ra, const double* __restrict__ dec, const
 }
 
 void launch_keys_pack(const double* ra, const double* dec, const int64_t* id, uint32_t n, GridView g, int passes,
-                      uint32_t* keys, Rec* rec, uint32_t* digit_hist, cudaStream_t s) {
+                      double r_max_arcsec, bool flagged, uint32_t* keys, Rec* rec, uint32_t* digit_hist, cudaStream_t s) {
     if (n == 0) return;
     int blocks = (int)std::min<size_t>(((size_t)n + kKeyThreads - 1) / kKeyThreads, (size_t)sm_count() * 8);
-    k_keys_pack<<<blocks, kKeyThreads, 0, s>>>(ra, dec, id, n, g, passes, keys, rec, digit_hist); count_launch();
+    const double rpad_deg = r_max_arcsec / 3600.0 + 1e-9;
+    const double sin_r = sin(r_max_arcsec * (M_PI / 648000.0)) * (1.0 + 1e-9);
+    k_keys_pack<<<blocks, kKeyThreads, 0, s>>>(ra, dec, id, n, g, passes, rpad_deg, sin_r, flagged ? 1 : 0, keys, rec, digit_hist);
+    count_launch();
 }
 
 // ------------------------------------------------------------------------------------------
@@ -377,7 +401,7 @@ void launch_gather(const Rec* rec, const uint32_t* perm, uint32_t n, double* x, 
 constexpr uint32_t kFillLane = 4, kFillWarp = 4096;
 
 __global__ void __launch_bounds__(256)
-k_cell_fill(const uint32_t* __restrict__ keys, uint32_t n, uint32_t n_cells, uint32_t* __restrict__ cell_start,
+k_cell_fill(const uint32_t* __restrict__ keys, uint32_t kmask, uint32_t n, uint32_t n_cells, uint32_t* __restrict__ cell_start,
             uint32_t* __restrict__ big, uint32_t* __restrict__ big_count, uint32_t big_cap) {
     __shared__ uint32_t s_keys[8][128];
     const int lane = threadIdx.x & 31;
@@ -391,13 +415,13 @@ k_cell_fill(const uint32_t* __restrict__ keys, uint32_t n, uint32_t n_cells, uin
         uint32_t k[4];
         if (i0 + 3 < n) {
             const uint4 v = __ldg(reinterpret_cast<const uint4*>(keys + i0));
-            k[0] = v.x; k[1] = v.y; k[2] = v.z; k[3] = v.w;
+            k[0] = v.x & kmask; k[1] = v.y & kmask; k[2] = v.z & kmask; k[3] = v.w & kmask;
         } else {
 #pragma unroll
-            for (int j = 0; j < 4; ++j) k[j] = i0 + j < n ? __ldg(keys + i0 + j) : n_cells;
+            for (int j = 0; j < 4; ++j) k[j] = i0 + j < n ? (__ldg(keys + i0 + j) & kmask) : n_cells;
         }
         uint32_t prev = __shfl_up_sync(0xffffffffu, k[3], 1);
-        if (lane == 0) prev = b > 0 ? __ldg(keys + b - 1) : 0u;
+        if (lane == 0) prev = b > 0 ? (__ldg(keys + b - 1) & kmask) : 0u;
         // common case, no long empty run inside the 128 rows: lanes own CELLS, not rows -- cell c gets the first row of
         // the step whose key is >= c (a binary search over the step's keys in shared memory), so the stores of a warp
         // are consecutive words instead of scattered ones
@@ -463,13 +487,13 @@ k_cell_fill_big(const uint32_t* __restrict__ big, const uint32_t* __restrict__ b
 
 size_t cell_big_cap(size_t n_cells) { return n_cells / kFillWarp + 2; }
 
-void launch_cell_table(const uint32_t* sorted_keys, uint32_t n, uint32_t n_cells, uint32_t* cell_start,
+void launch_cell_table(const uint32_t* sorted_keys, uint32_t key_mask, uint32_t n, uint32_t n_cells, uint32_t* cell_start,
                        uint32_t* d_big /*[3*cap + 1]*/, cudaStream_t s) {
     const uint32_t cap = (uint32_t)cell_big_cap(n_cells);
     uint32_t* d_count = d_big + 3 * (size_t)cap;
     cudaMemsetAsync(d_count, 0, sizeof(uint32_t), s);
     int blocks = (int)std::min<size_t>(((size_t)n + 1 + 1023) / 1024, (size_t)sm_count() * 16);
-    k_cell_fill<<<blocks, 256, 0, s>>>(sorted_keys, n, n_cells, cell_start, d_big, d_count, cap); count_launch();
+    k_cell_fill<<<blocks, 256, 0, s>>>(sorted_keys, key_mask, n, n_cells, cell_start, d_big, d_count, cap); count_launch();
     k_cell_fill_big<<<sm_count() * 4, 256, 0, s>>>(d_big, d_count, cap, cell_start); count_launch();
 }
 
@@ -499,7 +523,7 @@ k_zone_tiles(const uint32_t* __restrict__ cell_start, const uint32_t* __restrict
 
 __global__ void __launch_bounds__(256)
 k_tile_desc(const uint32_t* __restrict__ tile_first, uint32_t n_zones, const uint32_t* __restrict__ cell_start,
-            const uint32_t* __restrict__ cell_base, const uint32_t* __restrict__ keys, TileDesc* __restrict__ tiles) {
+            const uint32_t* __restrict__ cell_base, const uint32_t* __restrict__ keys, uint32_t kmask, TileDesc* __restrict__ tiles) {
     const uint32_t nt = __ldg(tile_first + n_zones);
     for (uint32_t t = blockIdx.x * 256 + threadIdx.x; t < nt; t += gridDim.x * 256) {
         uint32_t lo = 0, hi = n_zones;                // largest z with tile_first[z] <= t
@@ -510,17 +534,17 @@ k_tile_desc(const uint32_t* __restrict__ tile_first, uint32_t n_zones, const uin
         const uint32_t m = min((uint32_t)kTile, ze - s0);
         TileDesc d;
         d.first = s0; d.count = m; d.zone = z;
-        d.k_first = __ldg(keys + s0) - cb; d.k_last = __ldg(keys + s0 + m - 1) - cb;
+        d.k_first = (__ldg(keys + s0) & kmask) - cb; d.k_last = (__ldg(keys + s0 + m - 1) & kmask) - cb;
         d.pad0 = d.pad1 = d.pad2 = 0;
         tiles[t] = d;
     }
 }
 
 void launch_tiles(const uint32_t* cell_start, const uint32_t* cell_base, uint32_t n_zones, const uint32_t* sorted_keys,
-                  uint32_t tile_cap, uint32_t* d_tile_first, TileDesc* tiles, uint32_t* d_n_tiles, cudaStream_t s) {
+                  uint32_t key_mask, uint32_t tile_cap, uint32_t* d_tile_first, TileDesc* tiles, uint32_t* d_n_tiles, cudaStream_t s) {
     k_zone_tiles<<<1, 1024, 0, s>>>(cell_start, cell_base, n_zones, d_tile_first, d_n_tiles); count_launch();
     int blocks = (int)std::min<size_t>(((size_t)tile_cap + 255) / 256, (size_t)sm_count() * 8);
-    k_tile_desc<<<std::max(blocks, 1), 256, 0, s>>>(d_tile_first, n_zones, cell_start, cell_base, sorted_keys, tiles); count_launch();
+    k_tile_desc<<<std::max(blocks, 1), 256, 0, s>>>(d_tile_first, n_zones, cell_start, cell_base, sorted_keys, key_mask, tiles); count_launch();
 }
 
 }  // namespace hlc2

@@ -20,6 +20,16 @@ constexpr int kMaxPasses = 4;                 // 32-bit keys
 #endif
 constexpr int kTile = HLC2_TILE;                    // sources per match tile (= threads of the match CTA)
 
+// Window flags of a source on its own grid, kept in the top bits of its 32-bit cell key (grids of <= 2^28 cells).  They
+// say which cells of the source's OWN zone a search window of radius <= r_max can reach, so a match between two indices
+// that share one grid (opts.grid_like) needs no per-row window arithmetic:
+//   kKeyExtLo / kKeyExtHi  the window reaches into the previous / next RA cell of the zone
+//   kKeySlow               it leaves the zone (declination), passes RA = 0/360, or is wider than one cell (polar rows):
+//                          such rows take the general per-lane path
+constexpr int kKeyFlagShift = 28;
+constexpr uint32_t kKeyMask = (1u << kKeyFlagShift) - 1u;
+constexpr uint32_t kKeyExtLo = 1u << 28, kKeyExtHi = 1u << 29, kKeySlow = 1u << 30;
+
 // ---- grid as the kernels see it (passed by value) ----------------------------------------
 struct GridView {
     const int32_t* n_ra;        // [n_zones] RA cells per zone
@@ -45,6 +55,8 @@ struct IndexView {
     const double* x; const double* y; const double* z;   // [n] unit vectors, cell order
     const int64_t* id;                                    // [n]
     const float2* pos;                                    // [n] fp32 (ra, dec) estimate in degrees: locates windows, never decides
+    const uint32_t* key;                                  // [n] sorted cell keys (& key_mask), window flags in the top bits
+    uint32_t key_mask;                                    // kKeyMask when the keys carry flags, else 0xFFFFFFFF
     const uint32_t* cell_start;                           // [n_cells + 1]
     const TileDesc* tiles;                                // [*n_tiles]
     const uint32_t* n_tiles;                              // device scalar
@@ -71,7 +83,7 @@ int current_device();
 int sm_count();
 void launch_stats(const double* ra, const double* dec, uint32_t n, Stats* d_stats, cudaStream_t s);
 void launch_keys_pack(const double* ra, const double* dec, const int64_t* id, uint32_t n, GridView g, int passes,
-                      uint32_t* keys, Rec* rec, uint32_t* digit_hist, cudaStream_t s);
+                      double r_max_arcsec, bool flagged, uint32_t* keys, Rec* rec, uint32_t* digit_hist, cudaStream_t s);
 int  radix_passes(int key_bits);
 size_t sort_tiles(uint32_t n);
 // sorts (keys, row) by key; returns which of the double buffers holds the result (0 = a, 1 = b)
@@ -81,18 +93,19 @@ int  launch_radix_sort(uint32_t* keys_a, uint32_t* keys_b, uint32_t* val_a, uint
 void launch_gather(const Rec* rec, const uint32_t* perm, uint32_t n, double* x, double* y, double* z, int64_t* out_id,
                    float2* pos, cudaStream_t s);
 size_t cell_big_cap(size_t n_cells);
-void launch_cell_table(const uint32_t* sorted_keys, uint32_t n, uint32_t n_cells, uint32_t* cell_start,
+void launch_cell_table(const uint32_t* sorted_keys, uint32_t key_mask, uint32_t n, uint32_t n_cells, uint32_t* cell_start,
                        uint32_t* d_big, cudaStream_t s);
 void launch_tiles(const uint32_t* cell_start, const uint32_t* cell_base, uint32_t n_zones, const uint32_t* sorted_keys,
-                  uint32_t tile_cap, uint32_t* d_tile_first, TileDesc* tiles, uint32_t* d_n_tiles, cudaStream_t s);
+                  uint32_t key_mask, uint32_t tile_cap, uint32_t* d_tile_first, TileDesc* tiles, uint32_t* d_n_tiles, cudaStream_t s);
 
 size_t match_temp_bytes(const IndexView& A, const IndexView& B);
+constexpr uint32_t kMatchSameGrid = 1u;       // launch_match flag: A and B share one grid and both carry window flags
 size_t match_temp_for_tiles(size_t tile_cap);
 // upper bound of hlc2_crossmatch_sizes for any A index of <= n sources built with these options (hlc2_api.cu)
 size_t match_temp_bound(int64_t n_a, const hlc2_opts* opts);
 void launch_match(const IndexView& A, const IndexView& B, double radius_arcsec, int mode,
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
-                  unsigned long long* d_count, void* d_temp, cudaStream_t s,
+                  unsigned long long* d_count, void* d_temp, cudaStream_t s, uint32_t match_flags = 0,
                   cudaEvent_t ev_start = nullptr, cudaEvent_t ev_stop = nullptr);
 
 void count_launch(int k = 1);

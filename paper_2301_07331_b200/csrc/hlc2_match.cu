@@ -76,6 +76,8 @@ constexpr uint32_t kJobWrap = 1u << 10;      // window touches u = 0 / 360: rows
 constexpr uint32_t kJobFirst = 1u << 11;     // first / last job of its A tile (nearest mode carries the best across jobs)
 constexpr uint32_t kJobLast = 1u << 12;
 constexpr uint32_t kJobEnd = 1u << 13;       // producer -> consumers: no more work
+constexpr uint32_t kJobSame = 1u << 14;      // A and B share one grid: rows find their cells from their own key + window flags
+constexpr int kDqCap = 64;                   // rows a consumer warp holds back for the general path (drained 32 at a time)
 
 // 128-byte job record (32 words).  jobs[t] is the first job of A tile t; further jobs of a tile (windows that do
 // not fit one stage: the paper's calculation blocks, L253-257, cut to fit shared memory) are chained by `next`.
@@ -97,12 +99,12 @@ struct MatchArgs {
     uint32_t tile_cap, pool_cap;
 };
 
-struct SegDesc { double n_d; double centre; int32_t zone, k_lo, k_hi, cdelta; uint32_t rdelta, row_lo, row_hi, pad; };
-struct StageDesc { uint32_t a_first, a_count, a_off, flags; int32_t nseg; uint32_t pad; SegDesc seg[kSegs]; };
+struct SegDesc { double n_d; double centre; int32_t zone, k_lo, k_hi, cdelta; uint32_t rdelta, row_lo, row_hi; int32_t kbase; };
+struct StageDesc { uint32_t a_first, a_count, a_off, flags; int32_t nseg; uint32_t a_koff; SegDesc seg[kSegs]; };
 
 struct __align__(16) Stage {
     double ax[kAPad], ay[kAPad], az[kAPad];
-    float2 apos[kAPad];
+    float2 apos[kAPad];                                     // same-grid jobs: the rows' flagged cell keys (uint32) instead
     double bx[kBCap + 2], by[kBCap + 2], bz[kBCap + 2];     // slot kBCap: a point no chord test can reach
     uint32_t cs[kCsCap];
     StageDesc d;
@@ -113,6 +115,7 @@ struct WarpQueue { uint32_t a[kQCap], b[kQCap]; double c2[kQCap]; };
 struct __align__(16) MatchSmem {
     Stage st[kStages];
     WarpQueue q[kCW];
+    uint32_t dq[kCW][kDqCap];
     unsigned long long full[kStages], empty[kStages];
 };
 static_assert((kAPad * 8) % 16 == 0 && (kBCap * 8) % 16 == 0 && (kCsCap * 4) % 16 == 0, "bulk copies need 16-byte pieces");
@@ -223,6 +226,7 @@ __device__ __noinline__ void plan_piece(PlanState& st, const MatchArgs& p, const
     }
 }
 
+template <bool SAME>
 __global__ void __launch_bounds__(128)
 k_plan(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B, const __grid_constant__ MatchArgs p) {
     const uint32_t nt = __ldg(A.n_tiles);
@@ -245,7 +249,17 @@ k_plan(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B,
         const bool empty = qhi < gb.dec_min || qlo > gb.dec_max || t0.y == 0;
         bool direct = false;
         uint32_t common = 0;
-        if (!empty) {
+        if (SAME) {
+            // one grid for both catalogues: the rows of the tile sit in cells k_first..k_last of zone za, their window
+            // flags (index build) say which of them reach one cell further, and rows whose window leaves the zone are
+            // handled by the general path; so the tile's staged window is cells k_first-1 .. k_last+1 of the same zone
+            common = kJobSame;
+            if (t0.y != 0) {
+                const int n = __ldg(gb.n_ra + za);
+                plan_piece(st, p, B.cell_start, common, za, n, __ldg(gb.cell_base + za), max((int)t0.w - 1, 0), min((int)t1.x + 1, n - 1), 0.0f);
+                if (st.overflow) direct = true;
+            }
+        } else if (!empty) {
             const int zb0 = zone_of(gb, qlo), zb1 = zone_of(gb, qhi);
             if (zb1 - zb0 + 1 > kMaxZones) direct = true;
             const double cw = ga.span / (double)__ldg(ga.n_ra + za);
@@ -478,10 +492,23 @@ __device__ __forceinline__ void seg_ranges(const IndexView& A, const IndexView& 
     }
 }
 
+// rows of same-grid tiles whose window leaves their own zone (window flag kKeySlow): the general per-lane path, one
+// full warp of them at a time, from global memory (their tile was just staged, so the lines are in L2)
+template <int MODE>
+__device__ __noinline__ void drain_deferred(const IndexView& A, const IndexView& B, const MatchArgs& p, WarpQueue& q, unsigned& qn,
+                                            const uint32_t* dq, unsigned cnt, int lane) {
+    const bool act = (unsigned)lane < cnt;
+    const uint32_t a_row = act ? dq[lane] : 0u;
+    Best h; h.has = false; h.c2 = 0.0; h.row = 0;
+    if (act) scan_general<MODE>(A, B, p, a_row, __ldg(A.x + a_row), __ldg(A.y + a_row), __ldg(A.z + a_row), __ldg(A.pos + a_row), h);
+    __syncwarp();
+    if (MODE == HLC2_NEAREST) push_hits(A, B, p, q, qn, act && h.has, a_row, h.row, h.c2, lane);
+}
+
 // ------------------------------------------------------------------------------------------------------
 // k_match
 // ------------------------------------------------------------------------------------------------------
-template <int MODE>
+template <int MODE, bool SAME>
 __global__ void __launch_bounds__(kMatchThreads, HLC2_CTAS)
 k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B, const __grid_constant__ MatchArgs p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -541,18 +568,21 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
                 rtot += a; ctot += c;
             }
             const bool any = nseg != 0 || (flags & kJobDirect);
+            const bool same = SAME && (flags & kJobSame) != 0;
             const uint32_t a_al = a_first & ~1u;
             const uint32_t a_ld = any ? (((a_first + a_count + 1u) & ~1u) - a_al) : 0u;
-            const uint32_t bytes = a_ld * 32u + rtot * 24u + ctot * 4u;
+            const uint32_t k_al = a_first & ~3u;                                   // same-grid jobs stage 4-byte keys, not 8-byte pos
+            const uint32_t k_ld = any && same ? (((a_first + a_count + 3u) & ~3u) - k_al) : 0u;
+            const uint32_t bytes = a_ld * (same ? 24u : 32u) + k_ld * 4u + rtot * 24u + ctot * 4u;
 
             mbar_wait(&sm.empty[s], ph ^ 1u);
-            if (lane == 0) { st.d.a_first = a_first; st.d.a_count = a_count; st.d.a_off = a_first - a_al; st.d.flags = flags; st.d.nseg = nseg; }
+            if (lane == 0) { st.d.a_first = a_first; st.d.a_count = a_count; st.d.a_off = a_first - a_al; st.d.flags = flags; st.d.nseg = nseg; st.d.a_koff = a_first - k_al; }
             if (segact) {
                 SegDesc& e = st.d.seg[lane];
                 e.n_d = (double)(int32_t)n_ra; e.centre = (double)__uint_as_float(ctr);
                 e.zone = (int32_t)zone; e.k_lo = (int32_t)k_lo; e.k_hi = (int32_t)(k_lo + nk) - 1;
                 e.cdelta = (int32_t)((cs_lo - k_lo) - cs_al + coff); e.rdelta = roff - row_al;
-                e.row_lo = row_lo; e.row_hi = row_lo + nr;
+                e.row_lo = row_lo; e.row_hi = row_lo + nr; e.kbase = (int32_t)(cs_lo - k_lo);
             }
             __syncwarp();
             if (lane == 0) { if (bytes) mbar_arrive_expect_tx(&sm.full[s], bytes); else mbar_arrive(&sm.full[s]); }
@@ -565,9 +595,9 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
             if (a_ld && lane >= 8 && lane < 12) {
                 const int k = lane - 8;
                 const void* src = k == 0 ? (const void*)(A.x + a_al) : k == 1 ? (const void*)(A.y + a_al) : k == 2 ? (const void*)(A.z + a_al)
-                                : (const void*)(A.pos + a_al);
+                                : same ? (const void*)(A.key + k_al) : (const void*)(A.pos + a_al);
                 void* dst = k == 0 ? (void*)st.ax : k == 1 ? (void*)st.ay : k == 2 ? (void*)st.az : (void*)st.apos;
-                bulk_g2s(dst, src, a_ld * 8u, &sm.full[s]);
+                bulk_g2s(dst, src, k == 3 && same ? k_ld * 4u : a_ld * 8u, &sm.full[s]);
             }
             wcur = wnext; have = nhave;
         }
@@ -581,7 +611,8 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
     // ---------------- consumer warps: one lane per A row of the tile ----------------
     const GridView& g = B.g;
     WarpQueue& q = sm.q[warp];
-    unsigned qn = 0;
+    uint32_t* dq = sm.dq[warp];
+    unsigned qn = 0, dn = 0;
     Best best; best.has = false; best.c2 = 0.0; best.row = 0;
     for (uint32_t it = 0;; ++it) {
         const int s = (int)(it % kStages);
@@ -596,14 +627,38 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
             const bool act = threadIdx.x < a_count;
             if (MODE == HLC2_NEAREST && (flags & kJobFirst)) best.has = false;
             const uint32_t a_row = d.a_first + threadIdx.x;
-            if (nseg != 0 || (flags & kJobDirect)) {
+            if (SAME && (flags & kJobSame)) {
+                const unsigned ra = act ? threadIdx.x + d.a_off : d.a_off;
+                const double ax = st.ax[ra], ay = st.ay[ra], az = st.az[ra];
+                const uint32_t kf = reinterpret_cast<const uint32_t*>(st.apos)[(act ? threadIdx.x : 0u) + d.a_koff];
+                const bool slow = (kf & kKeySlow) != 0;
+                if (flags & kJobFirst) {            // rows whose window leaves their zone: held back for the general path, once per tile
+                    const unsigned m = __ballot_sync(kFull, act && slow);
+                    if (m) {
+                        if (act && slow) dq[dn + __popc(m & ((1u << lane) - 1u))] = a_row;
+                        dn += __popc(m);
+                    }
+                }
+                const int klo = (int)(kf & kKeyMask) - (int)((kf >> kKeyFlagShift) & 1u);
+                const int khi = (int)(kf & kKeyMask) + (int)((kf >> (kKeyFlagShift + 1)) & 1u);
+                for (int sg = 0; sg < nseg; ++sg) {
+                    const SegDesc& e = d.seg[sg];
+                    const int k0 = max(klo - e.kbase, e.k_lo), k1 = min(khi - e.kbase, e.k_hi);     // zone-local cells, clipped to the piece
+                    unsigned q0 = 0, q1 = 0;
+                    if (act && !slow && k0 <= k1) {
+                        q0 = min(max(st.cs[k0 + e.cdelta], e.row_lo), e.row_hi) + e.rdelta;
+                        q1 = min(max(st.cs[k1 + 1 + e.cdelta], e.row_lo), e.row_hi) + e.rdelta;
+                    }
+                    scan_staged<MODE>(A, B, st, p, q, qn, a_row, ax, ay, az, q0, q1, e.rdelta, best, lane);
+                }
+            } else if (nseg != 0 || (flags & kJobDirect)) {
                 const unsigned ra = act ? threadIdx.x + d.a_off : d.a_off;
                 const double ax = st.ax[ra], ay = st.ay[ra], az = st.az[ra];
                 const float2 pf = st.apos[ra];
                 if (flags & kJobDirect) {
                     if (act) scan_general<MODE>(A, B, p, a_row, ax, ay, az, pf, best);
                     __syncwarp();
-                } else {
+                } else if (!SAME) {
                     const double dlo = (double)pf.y - p.pad_dec, dhi = (double)pf.y + p.pad_dec;
                     const int zlo = zone_of(g, dlo), zhi = zone_of(g, dhi);
                     const float fx = (float)ax, fy = (float)ay;
@@ -624,8 +679,17 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm.empty[s]);
+        if (SAME && dn >= 32u) {                    // a full warp of held-back rows: general path, off the stage
+            drain_deferred<MODE>(A, B, p, q, qn, dq, 32u, lane);
+            const uint32_t v = lane + 32u < dn ? dq[lane + 32u] : 0u;
+            __syncwarp();
+            if (lane + 32u < dn) dq[lane] = v;
+            dn -= 32u;
+            __syncwarp();
+        }
     }
     __syncwarp();
+    if (SAME && dn) drain_deferred<MODE>(A, B, p, q, qn, dq, dn, lane);
     if (qn) flush_rows(A, B, p, q, 0, qn, lane);
 }
 
@@ -636,7 +700,8 @@ size_t match_temp_bytes(const IndexView& A, const IndexView& B) { return match_t
 
 void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_arcsec, int mode,
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
-                  unsigned long long* d_count, void* d_temp, cudaStream_t s, cudaEvent_t ev_start, cudaEvent_t ev_stop) {
+                  unsigned long long* d_count, void* d_temp, cudaStream_t s, uint32_t match_flags,
+                  cudaEvent_t ev_start, cudaEvent_t ev_stop) {
     if (A_in.n == 0 || B_in.n == 0) {
         if (ev_start) cudaEventRecord(ev_start, s);
         if (ev_stop) cudaEventRecord(ev_stop, s);
@@ -664,29 +729,28 @@ void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_ar
     p.jobs = reinterpret_cast<Job*>(reinterpret_cast<char*>(d_temp) + 256);
     p.tile_cap = (uint32_t)tiles; p.pool_cap = (uint32_t)pool_cap_of(tiles);
     cudaMemsetAsync(p.pool_count, 0, sizeof(uint32_t), s);
-    const int m = mode == HLC2_NEAREST ? 1 : 0;
-    static int per_sm_dev[kMaxDevices][2] = {};        // resident CTAs per SM; the smem opt-in is per device
+    const bool same = (match_flags & kMatchSameGrid) != 0;
+    const int m = (mode == HLC2_NEAREST ? 1 : 0) + (same ? 2 : 0);
+    const void* kern = m == 0 ? (const void*)k_match<HLC2_ALL_PAIRS, false> : m == 1 ? (const void*)k_match<HLC2_NEAREST, false>
+                     : m == 2 ? (const void*)k_match<HLC2_ALL_PAIRS, true> : (const void*)k_match<HLC2_NEAREST, true>;
+    static int per_sm_dev[kMaxDevices][4] = {};        // resident CTAs per SM; the smem opt-in is per device
     int* per_sm = per_sm_dev[current_device()];
     const size_t smem = sizeof(MatchSmem);
     if (!per_sm[m]) {
         int v = 0;
-        if (m) {
-            cudaFuncSetAttribute(k_match<HLC2_NEAREST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_match<HLC2_NEAREST>, kMatchThreads, smem);
-        } else {
-            cudaFuncSetAttribute(k_match<HLC2_ALL_PAIRS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, k_match<HLC2_ALL_PAIRS>, kMatchThreads, smem);
-        }
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, kern, kMatchThreads, smem);
         per_sm[m] = v > 0 ? v : 1;
     }
     const unsigned pblocks = (unsigned)std::min<size_t>((tiles + 127) / 128, (size_t)sm_count() * 8);
-    k_plan<<<pblocks, 128, 0, s>>>(A, B, p);
+    if (same) k_plan<true><<<pblocks, 128, 0, s>>>(A, B, p);
+    else                              k_plan<false><<<pblocks, 128, 0, s>>>(A, B, p);
     count_launch();
     // persistent grid: SM count x resident CTAs, never more CTAs than tiles
     const unsigned blocks = (unsigned)std::max<size_t>(1, std::min<size_t>(tiles, (size_t)sm_count() * per_sm[m]));
     if (ev_start) cudaEventRecord(ev_start, s);          // the caller's events bracket k_match alone (hlc2_crossmatch_events)
-    if (m) k_match<HLC2_NEAREST><<<blocks, kMatchThreads, smem, s>>>(A, B, p);
-    else   k_match<HLC2_ALL_PAIRS><<<blocks, kMatchThreads, smem, s>>>(A, B, p);
+    void* kargs[3] = {(void*)&A, (void*)&B, (void*)&p};
+    cudaLaunchKernel(kern, dim3(blocks), dim3(kMatchThreads), kargs, smem, s);
     count_launch();
     if (ev_stop) cudaEventRecord(ev_stop, s);
 }

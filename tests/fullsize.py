@@ -146,7 +146,7 @@ def stratified_subsample(w, grid, m=200_000, seed=4):
     return np.sort(np.concatenate(rows))
 
 
-def report(P, cfg, scale=1.0, one_core=False, same_grid=False, out_dir=None):
+def report(P, cfg, scale=1.0, one_core=False, same_grid=False, out_dir=None, brute_rows=200_000):
     """Run configuration `cfg` at `scale` (1.0 = the stated size) and compare every mode with the oracle."""
     import torch
     t0 = time.perf_counter()
@@ -154,6 +154,8 @@ def report(P, cfg, scale=1.0, one_core=False, same_grid=False, out_dir=None):
     if cfg == 4:
         w, like_b, grid = cfg4_workload(P, scale)
         opts_a = P.make_opts(3.0, cell_arcsec=160.0, full_sky=True); opts_b = P.make_opts(3.0)
+        if same_grid:
+            opts_a = P.make_opts(3.0)
     else:
         w = S.config(cfg, scale=scale)
         opts_a = opts_b = P.make_opts(w.radius_arcsec)
@@ -183,7 +185,7 @@ def report(P, cfg, scale=1.0, one_core=False, same_grid=False, out_dir=None):
             rep["oracle_seconds_1core"] = time.perf_counter() - t1
         if cfg == 4 and mode == P.HLC2_ALL_PAIRS:
             # the prescribed completeness check: brute force ("No Index") on a stratified subsample of A
-            rows = stratified_subsample(w, grid, min(200_000, len(w.A)))
+            rows = stratified_subsample(w, grid, min(brute_rows, len(w.A)))
             sub = w.A.take(rows)
             t1 = time.perf_counter()
             ba, bb, bs, _ = oracle.match(sub.ra, sub.dec, sub.id, w.B.ra, w.B.dec, w.B.id, r, mode, oracle.ENGINE_BRUTE)

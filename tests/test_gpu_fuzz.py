@@ -59,9 +59,19 @@ def test_random_geometry_parity(P, seed):
     A, B, r = make_case(seed)
     dev = lambda c: (torch.from_numpy(c.ra).cuda(), torch.from_numpy(c.dec).cuda(), torch.from_numpy(c.id).cuda())
     ia = P.hlc2_build_index(*dev(A), opts=P.make_opts(r)); ib = P.hlc2_build_index(*dev(B), opts=P.make_opts(r))
+    # A filed on B's grid as well (the same-grid path), when A fits inside B's RA box
+    try:
+        ia_same = P.hlc2_build_index(*dev(A), opts=P.make_opts(r), like=ib)
+    except P.Hlc2Error as e:
+        assert e.status == P.HLC2_ERR_GRID_MISMATCH
+        ia_same = None
+    sep_of = parity.make_sep_of(A, B)
     for mode in (0, 1):
-        a, b, s = P.crossmatch(ia, ib, r, mode, capacity=max(1024, 4 * max(len(A), len(B))))
         oa, ob, os_, _ = oracle.match(A.ra, A.dec, A.id, B.ra, B.dec, B.id, r, mode)
         cmp = parity.compare_nearest if mode else parity.compare_all_pairs
-        rep = cmp((a.cpu().numpy(), b.cpu().numpy(), s.cpu().numpy()), (oa, ob, os_), r, parity.make_sep_of(A, B))
-        assert len(rep["borderline"]) <= 2
+        for ixa in (ia, ia_same):
+            if ixa is None:
+                continue
+            a, b, s = P.crossmatch(ixa, ib, r, mode, capacity=max(1024, 4 * max(len(A), len(B))))
+            rep = cmp((a.cpu().numpy(), b.cpu().numpy(), s.cpu().numpy()), (oa, ob, os_), r, sep_of)
+            assert len(rep["borderline"]) <= 2

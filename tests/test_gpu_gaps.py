@@ -129,7 +129,7 @@ def test_job_pool_overflow_falls_back(P, mode):
     P.hlc2_crossmatch(ia, ib, 5.0, mode, oa, ob, os_, cnt, temp=temp)
     n = int(cnt.item()); assert n <= cap
     pool_n = int(temp[:4].view(torch.int32).item())
-    pool_cap = (need - 256) // 128 - (len(A) // 128 + P.hlc2_grid_describe(ia)["n_zones"] + 1)
+    pool_cap = 3 * (len(A) // 128 + P.hlc2_grid_describe(ia)["n_zones"] + 1) + 4096        # of the driving catalogue's tiles
     assert pool_n > pool_cap, (pool_n, pool_cap)          # the counter ran past the pool: the overflow branch was taken
     oa_, ob_, os2, _ = oracle.match(A.ra, A.dec, A.id, B.ra, B.dec, B.id, 5.0, mode)
     cmp = parity.compare_nearest if mode else parity.compare_all_pairs

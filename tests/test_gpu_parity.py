@@ -30,9 +30,9 @@ def dev(cat):
     return (torch.from_numpy(cat.ra).cuda(), torch.from_numpy(cat.dec).cuda(), torch.from_numpy(cat.id).cuda())
 
 
-def gpu_match(P, A, B, radius, mode, opts_a=None, opts_b=None, **kw):
-    ia = P.hlc2_build_index(*dev(A), opts=opts_a or P.make_opts(radius, **kw))
+def gpu_match(P, A, B, radius, mode, opts_a=None, opts_b=None, same_grid=False, **kw):
     ib = P.hlc2_build_index(*dev(B), opts=opts_b or P.make_opts(radius, **kw))
+    ia = P.hlc2_build_index(*dev(A), opts=opts_a or P.make_opts(radius, **kw), like=ib if same_grid else None)
     assert P.hlc2_index_status(ia)[0] == 0 and P.hlc2_index_status(ib)[0] == 0
     a, b, s = P.crossmatch(ia, ib, radius, mode)
     return a.cpu().numpy(), b.cpu().numpy(), s.cpu().numpy(), ia, ib
@@ -61,6 +61,9 @@ def test_index_invariants(P, cfg, scale):
     n, nc = arr["n"], arr["n_cells"]
     assert n == len(w.B)
     key = arr["cell_key"].cpu().numpy().view(np.uint32).astype(np.int64)
+    flags = key >> 28                                  # window flags ride in the top bits (include/hlc2.h, HLC2_KEY_MASK)
+    key = key & P.HLC2_KEY_MASK
+    assert flags.max() <= 4 and ((flags & 4 == 0) | (flags == 4)).all()
     cs = arr["cell_start"].cpu().numpy().view(np.uint32).astype(np.int64)
     assert (np.diff(key) >= 0).all() and key.max() < nc
     assert cs[0] == 0 and cs[-1] == n and (np.diff(cs) >= 0).all()
@@ -86,22 +89,27 @@ def test_cfg1_tiny_patch(P, mode):
     m = P.HLC2_NEAREST if mode == "nearest" else P.HLC2_ALL_PAIRS
     rep, _, _ = check(P, w.A, w.B, w.radius_arcsec, m)
     assert rep["n_gpu"] > 75_000
-    # the same patch matched with cells forced to the minimum size (= r) and with huge cells
+    # the same patch matched with cells forced to the minimum size (= r) and with huge cells, each also with A filed
+    # on B's grid (opts.grid_like: the same-grid path of the match)
+    check(P, w.A, w.B, w.radius_arcsec, m, same_grid=True)
     for cell in (1.0, 900.0):
         check(P, w.A, w.B, w.radius_arcsec, m, cell_arcsec=cell)
+        check(P, w.A, w.B, w.radius_arcsec, m, cell_arcsec=cell, same_grid=True)
 
 
+@pytest.mark.parametrize("same_grid", [False, True])
 @pytest.mark.parametrize("mode", ["all_pairs", "nearest"])
-def test_cfg2_full_sky_scaled(P, mode):
+def test_cfg2_full_sky_scaled(P, mode, same_grid):
     w = S.config(2, scale=0.1)          # 1e6 x 1e6: several hundred tiles and a ragged tail
     m = P.HLC2_NEAREST if mode == "nearest" else P.HLC2_ALL_PAIRS
-    rep, _, _ = check(P, w.A, w.B, w.radius_arcsec, m)
+    rep, _, _ = check(P, w.A, w.B, w.radius_arcsec, m, same_grid=same_grid)
     assert rep["n_gpu"] > 690_000
 
 
-def test_cfg3_gaia_like_scaled(P):
+@pytest.mark.parametrize("same_grid", [False, True])
+def test_cfg3_gaia_like_scaled(P, same_grid):
     w = S.config(3, scale=0.012)        # 1.2e6 x 6e5, galactic-plane density contrast
-    rep, _, _ = check(P, w.A, w.B, w.radius_arcsec, P.HLC2_ALL_PAIRS)
+    rep, _, _ = check(P, w.A, w.B, w.radius_arcsec, P.HLC2_ALL_PAIRS, same_grid=same_grid)
     assert rep["n_gpu"] > 355_000
 
 
@@ -120,12 +128,15 @@ def test_cfg4_boundary_stress_vs_brute_force(P):
     ib = P.hlc2_build_index(*dev(w.B), opts=P.make_opts(3.0), like=pre)          # exactly the described grid
     gb_grid = P.hlc2_grid_describe(ib)
     assert gb_grid["n_cells"] == grid["n_cells"] and np.array_equal(gb_grid["n_ra"], grid["n_ra"])
+    ia_same = P.hlc2_build_index(*dev(w.A), opts=P.make_opts(3.0), like=pre)     # A on the same grid: the same-grid path
+    sep_of = parity.make_sep_of(w.A, w.B)
     for mode in (P.HLC2_ALL_PAIRS, P.HLC2_NEAREST):
-        a, b, s = P.crossmatch(ia, ib, 3.0, mode)
         oa, ob, os_, _ = oracle.match(w.A.ra, w.A.dec, w.A.id, w.B.ra, w.B.dec, w.B.id, 3.0, mode, oracle.ENGINE_BRUTE)
         cmp = parity.compare_nearest if mode == P.HLC2_NEAREST else parity.compare_all_pairs
-        rep = cmp((a.cpu().numpy(), b.cpu().numpy(), s.cpu().numpy()), (oa, ob, os_), 3.0, parity.make_sep_of(w.A, w.B))
-        assert rep["n_oracle"] > 150_000 and len(rep["borderline"]) <= 2
+        for ixa in (ia, ia_same):
+            a, b, s = P.crossmatch(ixa, ib, 3.0, mode)
+            rep = cmp((a.cpu().numpy(), b.cpu().numpy(), s.cpu().numpy()), (oa, ob, os_), 3.0, sep_of)
+            assert rep["n_oracle"] > 150_000 and len(rep["borderline"]) <= 2
 
 
 # ------------------------------------------------------------------------------ poles, seam, degenerate inputs
@@ -150,6 +161,7 @@ def test_poles_seam_duplicates_micro(P, radius, mode):
     A, B = _tiny()
     for kw in ({}, {"full_sky": True}, {"cell_arcsec": radius}, {"cell_arcsec": 20000.0}):
         check(P, A, B, radius, mode, engine=oracle.ENGINE_BRUTE_LD, **kw)
+        check(P, A, B, radius, mode, engine=oracle.ENGINE_BRUTE_LD, same_grid=True, **kw)
 
 
 def test_patch_across_ra_seam_and_on_pole(P):
