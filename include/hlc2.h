@@ -74,6 +74,11 @@ typedef enum {
  *                     (max(r_max, sqrt(target_occupancy * occupied area / n))).  Honoured while the cell
  *                     table stays within max(16 n, 2^25) cells, else coarsened until it fits.
  *   full_sky          non-zero: the grid spans the whole sphere whatever the data extent.
+ *   zone_aspect       zones are zone_aspect times as high as the fine-cell size and RA cells that much narrower (same
+ *                     cell area, both never below r_max): a source's search window then leaves its zone zone_aspect times
+ *                     less often and reaches a neighbouring RA cell that much more often -- the second is the cheap one
+ *                     (one more cell of the same contiguous row range).  0 -> automatic: min(32, floor(cell / (3 r_max))), at
+ *                     least 1; 1 = square cells.
  *   grid_like         if non-NULL, reuse that index's grid exactly (zones, cells, box).  The
  *                     catalogue must lie inside that grid's box (else HLC2_ERR_GRID_MISMATCH).
  */
@@ -82,7 +87,7 @@ typedef struct {
     double target_occupancy;
     double cell_arcsec;
     int32_t full_sky;
-    int32_t reserved;
+    int32_t zone_aspect;
     const hlc2_index* grid_like;
 } hlc2_opts;
 

@@ -46,7 +46,7 @@ class Hlc2Error(RuntimeError):
 
 class hlc2_opts(ctypes.Structure):
     _fields_ = [("r_max_arcsec", ctypes.c_double), ("target_occupancy", ctypes.c_double),
-                ("cell_arcsec", ctypes.c_double), ("full_sky", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("cell_arcsec", ctypes.c_double), ("full_sky", ctypes.c_int32), ("zone_aspect", ctypes.c_int32),
                 ("grid_like", ctypes.c_void_p)]
 
 
@@ -101,10 +101,10 @@ def _stream_ptr(stream):
     return ctypes.c_void_p(s.cuda_stream)
 
 
-def make_opts(r_max_arcsec=1.0, target_occupancy=0.0, cell_arcsec=0.0, full_sky=False, grid_like=None) -> hlc2_opts:
+def make_opts(r_max_arcsec=1.0, target_occupancy=0.0, cell_arcsec=0.0, full_sky=False, grid_like=None, zone_aspect=0) -> hlc2_opts:
     o = hlc2_opts()
     o.r_max_arcsec = float(r_max_arcsec); o.target_occupancy = float(target_occupancy)
-    o.cell_arcsec = float(cell_arcsec); o.full_sky = int(bool(full_sky)); o.reserved = 0
+    o.cell_arcsec = float(cell_arcsec); o.full_sky = int(bool(full_sky)); o.zone_aspect = int(zone_aspect)
     o.grid_like = grid_like.handle if grid_like is not None else None
     return o
 

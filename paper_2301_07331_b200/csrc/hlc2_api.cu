@@ -65,6 +65,7 @@ static bool opts_ok(const hlc2_opts* o) {
     if (!(o->target_occupancy >= 0.0) || !std::isfinite(o->target_occupancy)) return false;
     if (!(o->cell_arcsec >= 0.0) || !std::isfinite(o->cell_arcsec)) return false;
     if (o->grid_like && o->grid_like->magic != kMagic) return false;
+    if (o->zone_aspect < 0 || o->zone_aspect > 64) return false;
     return true;
 }
 // target_occupancy 0 = automatic: cells as fine as the radix sort allows for free.  Finer cells of the scanned
@@ -147,7 +148,7 @@ size_t match_temp_bound(int64_t n_a, const hlc2_opts* opts) {
     hlc2_opts o = opts_or_default(opts, n_a);
     o.grid_like = nullptr;
     Layout L = make_layout(n_a, o);
-    return match_temp_for_tiles(L.cap_tiles);
+    return std::max(match_temp_for_tiles(L.cap_tiles), (size_t)256 + (size_t)n_a * sizeof(uint32_t));
 }
 }  // namespace hlc2
 
@@ -201,12 +202,17 @@ static void plan_grid(const Stats& st, int64_t n_valid, const hlc2_opts& o, size
     c = std::max(c, o.r_max_arcsec);
     c = std::min(c, 648000.0);
     for (int iter = 0; iter < 2000; ++iter) {
-        double c_deg = c / 3600.0;
-        double rng = std::max(range, c_deg);
-        int64_t nz = std::max<int64_t>(1, (int64_t)floor(rng / c_deg));
+        // zones `aspect` times as high as the cell size, RA cells that much narrower (never below r_max): same cell area,
+        // but a search window leaves its zone (the expensive neighbour) aspect times less often
+        // automatic: RA cells three r_max wide (measured on config 3: the match time falls until about there)
+        const double want = o.zone_aspect > 0 ? (double)o.zone_aspect : std::min(32.0, floor(c / (3.0 * o.r_max_arcsec)));
+        const double aspect = std::max(1.0, std::min(want, c / o.r_max_arcsec));
+        double zh_deg = std::min(c * aspect, 648000.0) / 3600.0;
+        double rng = std::max(range, zh_deg);
+        int64_t nz = std::max<int64_t>(1, (int64_t)floor(rng / zh_deg));
         g.n_zones = nz; g.h = rng / (double)nz; g.dec_lo = dec_lo; g.cell_arcsec = c;
         if ((size_t)nz <= cap_zones) {
-            fill_zones(g, c);
+            fill_zones(g, c / aspect);
             uint64_t tot = 0; for (int32_t k : g.n_ra) tot += (uint64_t)k;
             if (tot <= cap_cells && tot < 0xFFFFFFF0ull) return;
         }
@@ -236,11 +242,14 @@ static IndexView index_view(const hlc2_index* ix) {
     return v;
 }
 
-// do two indices share one grid (same zones, same cells, same box)?  Then a source's cell key means the same in both.
+// do two indices share one grid (same zones, same cells, same box)?  Then a source's cell key means the same in both and
+// A's window flags select its cells (hlc2_match_same.cu).  That path hands every row within r_max of a zone edge to
+// its per-lane edge kernel, which pays off while such rows are few: zones at least 4 r_max high (else the general
+// path, which stages all three zones, is the better one).
 static bool same_grid(const hlc2_index* a, const hlc2_index* b) {
     const HostGrid& x = a->grid; const HostGrid& y = b->grid;
     return a->flagged && b->flagged && x.n_zones == y.n_zones && x.dec_lo == y.dec_lo && x.h == y.h && x.ra0 == y.ra0 &&
-           x.span == y.span && x.n_ra == y.n_ra;
+           x.span == y.span && x.n_ra == y.n_ra && 4.0 * a->opts.r_max_arcsec / 3600.0 <= x.h;
 }
 
 // does every occupied coarse RA bin of `st` lie inside grid g's RA box?
@@ -336,7 +345,7 @@ int hlc2_build_index(const double* d_ra, const double* d_dec, const int64_t* d_i
     const uint32_t* perm = where ? pb : pa;
     launch_gather(rec, perm, nn, (double*)(buf + L.x), (double*)(buf + L.y), (double*)(buf + L.z), (int64_t*)(buf + L.id), (float2*)(buf + L.pos), s);
     launch_cell_table(key_idx, kmask, nn, n_cells, (uint32_t*)(buf + L.cell_start), (uint32_t*)(tmp + T.big), s);
-    launch_tiles((const uint32_t*)(buf + L.cell_start), gv.cell_base, (uint32_t)g.n_zones, key_idx, kmask,
+    launch_tiles((const uint32_t*)(buf + L.cell_start), gv.cell_base, gv.n_ra, (uint32_t)g.n_zones, key_idx, kmask,
                  (uint32_t)((size_t)n / kTile + (size_t)g.n_zones + 1), (uint32_t*)(tmp + T.tile_first),
                  (TileDesc*)(buf + L.tiles), (uint32_t*)(buf + L.n_tiles), s);
     cudaError_t e = cudaGetLastError();

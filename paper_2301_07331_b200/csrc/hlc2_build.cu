@@ -131,21 +131,22 @@ __device__ __forceinline__ void unit_vector(double ra_norm, double dec, double& 
 
 constexpr int kKeyThreads = 256;
 
-// Window flags of a valid source on its own grid (see kKeyExtLo / kKeyExtHi / kKeySlow).  Any source within r_max of
+// Window flags of a valid source on its own grid (see kKeyExtLo ... kKeyGeneral).  Any source within r_max of
 // this one has a declination in [dec - r, dec + r] and an RA within asin(sin r / cos dec) of it, and zone_of / cell_of_u
 // are monotone, so its zone and cell lie between those of the window's ends evaluated with the SAME expressions that
 // file sources: flags computed from the padded window are a superset of what any query radius <= r_max needs.
 __device__ __forceinline__ uint32_t window_flags(const GridView& g, double dec, double cd, double u, int z, int nra, int k,
                                                  double rpad_deg, double sin_r) {
-    if (zone_of(g, dec - rpad_deg) != z || zone_of(g, dec + rpad_deg) != z) return kKeySlow;
+    const int zl = zone_of(g, dec - rpad_deg), zh = zone_of(g, dec + rpad_deg);
+    if (zl < z - 1 || zh > z + 1) return kKeyGeneral;
     const double s = sin_r / fmax(cd, 1e-300);                       // sin of the RA half-window
-    if (!(s < 0.2)) return kKeySlow;                                  // polar rows: wide windows, rings
+    if (!(s < 0.2)) return kKeyGeneral;                               // polar rows: wide windows, rings
     const double w = fma(0.2 * s * s, s, s) * 57.29577951308232 + 1e-9;   // asin(s) <= s + s^3 / 5 below 0.2
     const double ulo = u - w, uhi = u + w;
-    if (ulo < 0.0 ? ulo + 360.0 <= g.span : uhi >= 360.0) return kKeySlow;  // the window's image through RA = 0/360 lies inside the box
+    if (ulo < 0.0 ? ulo + 360.0 <= g.span : uhi >= 360.0) return kKeyGeneral;  // the window's image through RA = 0/360 lies inside the box
     const int klo = cell_of_u(g, fmax(ulo, 0.0), nra), khi = cell_of_u(g, fmin(uhi, g.span), nra);
-    if (klo < k - 1 || khi > k + 1) return kKeySlow;
-    return (klo < k ? kKeyExtLo : 0u) | (khi > k ? kKeyExtHi : 0u);
+    if (klo < k - 1 || khi > k + 1) return kKeyGeneral;
+    return (klo < k ? kKeyExtLo : 0u) | (khi > k ? kKeyExtHi : 0u) | (zl < z ? kKeyDecLo : 0u) | (zh > z ? kKeyDecHi : 0u);
 }
 
 __global__ void __launch_bounds__(kKeyThreads)
@@ -521,30 +522,44 @@ k_zone_tiles(const uint32_t* __restrict__ cell_start, const uint32_t* __restrict
     if (threadIdx.x == 0) { tile_first[n_zones] = carry; *n_tiles = carry; }
 }
 
+// one warp per tile: descriptor + the OR of the rows' window flags (so the same-grid match knows without looking at
+// the rows whether any of them reaches into the zone below / above or needs the general path)
 __global__ void __launch_bounds__(256)
 k_tile_desc(const uint32_t* __restrict__ tile_first, uint32_t n_zones, const uint32_t* __restrict__ cell_start,
-            const uint32_t* __restrict__ cell_base, const uint32_t* __restrict__ keys, uint32_t kmask, TileDesc* __restrict__ tiles) {
+            const uint32_t* __restrict__ cell_base, const uint32_t* __restrict__ n_ra, const uint32_t* __restrict__ keys, uint32_t kmask,
+            TileDesc* __restrict__ tiles) {
     const uint32_t nt = __ldg(tile_first + n_zones);
-    for (uint32_t t = blockIdx.x * 256 + threadIdx.x; t < nt; t += gridDim.x * 256) {
+    const int lane = threadIdx.x & 31;
+    for (uint32_t t = blockIdx.x * 8 + (threadIdx.x >> 5); t < nt; t += gridDim.x * 8) {
         uint32_t lo = 0, hi = n_zones;                // largest z with tile_first[z] <= t
         while (hi - lo > 1) { uint32_t mid = (lo + hi) >> 1; if (__ldg(tile_first + mid) <= t) lo = mid; else hi = mid; }
         const uint32_t z = lo, cb = __ldg(cell_base + z);
         const uint32_t zs = __ldg(cell_start + cb), ze = __ldg(cell_start + __ldg(cell_base + z + 1));
         const uint32_t s0 = zs + (t - __ldg(tile_first + z)) * kTile;
         const uint32_t m = min((uint32_t)kTile, ze - s0);
-        TileDesc d;
-        d.first = s0; d.count = m; d.zone = z;
-        d.k_first = (__ldg(keys + s0) & kmask) - cb; d.k_last = (__ldg(keys + s0 + m - 1) & kmask) - cb;
-        d.pad0 = d.pad1 = d.pad2 = 0;
-        tiles[t] = d;
+        uint32_t fl = 0;
+        for (uint32_t i = lane; i < m; i += 32) {
+            const uint32_t f = __ldg(keys + s0 + i) & ~kmask;
+            fl |= (f & kKeyGeneral) == kKeyGeneral ? kTileGeneral : ((f & kKeyDecLo ? kTileDecLo : 0u) | (f & kKeyDecHi ? kTileDecHi : 0u));
+        }
+        fl = __reduce_or_sync(0xffffffffu, fl);
+        if (lane == 0) {
+            TileDesc d;
+            d.first = s0; d.count = m; d.zone = z;
+            d.k_first = (__ldg(keys + s0) & kmask) - cb; d.k_last = (__ldg(keys + s0 + m - 1) & kmask) - cb;
+            d.flags = fl; d.cb = cb;
+            d.n = __ldg(n_ra + z); d.n_lo = z > 0 ? __ldg(n_ra + z - 1) : 0u; d.n_hi = z + 1 < n_zones ? __ldg(n_ra + z + 1) : 0u;
+            d.inv_n = 1.0 / (double)d.n;
+            tiles[t] = d;
+        }
     }
 }
 
-void launch_tiles(const uint32_t* cell_start, const uint32_t* cell_base, uint32_t n_zones, const uint32_t* sorted_keys,
+void launch_tiles(const uint32_t* cell_start, const uint32_t* cell_base, const int32_t* n_ra, uint32_t n_zones, const uint32_t* sorted_keys,
                   uint32_t key_mask, uint32_t tile_cap, uint32_t* d_tile_first, TileDesc* tiles, uint32_t* d_n_tiles, cudaStream_t s) {
     k_zone_tiles<<<1, 1024, 0, s>>>(cell_start, cell_base, n_zones, d_tile_first, d_n_tiles); count_launch();
-    int blocks = (int)std::min<size_t>(((size_t)tile_cap + 255) / 256, (size_t)sm_count() * 8);
-    k_tile_desc<<<std::max(blocks, 1), 256, 0, s>>>(d_tile_first, n_zones, cell_start, cell_base, sorted_keys, key_mask, tiles); count_launch();
+    int blocks = (int)std::min<size_t>(((size_t)tile_cap + 7) / 8, (size_t)sm_count() * 8);
+    k_tile_desc<<<std::max(blocks, 1), 256, 0, s>>>(d_tile_first, n_zones, cell_start, cell_base, reinterpret_cast<const uint32_t*>(n_ra), sorted_keys, key_mask, tiles); count_launch();
 }
 
 }  // namespace hlc2

@@ -21,14 +21,16 @@ constexpr int kMaxPasses = 4;                 // 32-bit keys
 constexpr int kTile = HLC2_TILE;                    // sources per match tile (= threads of the match CTA)
 
 // Window flags of a source on its own grid, kept in the top bits of its 32-bit cell key (grids of <= 2^28 cells).  They
-// say which cells of the source's OWN zone a search window of radius <= r_max can reach, so a match between two indices
-// that share one grid (opts.grid_like) needs no per-row window arithmetic:
-//   kKeyExtLo / kKeyExtHi  the window reaches into the previous / next RA cell of the zone
-//   kKeySlow               it leaves the zone (declination), passes RA = 0/360, or is wider than one cell (polar rows):
-//                          such rows take the general per-lane path
+// say which cells around the source's own cell a search window of radius <= r_max can reach, so a match between two
+// indices that share one grid (opts.grid_like) needs no per-row window arithmetic:
+//   kKeyExtLo / kKeyExtHi  the window reaches into the previous / next RA cell of the source's zone
+//   kKeyDecLo / kKeyDecHi  it reaches into the zone below / above (never further: zones are at least r_max high)
+//   kKeyGeneral (both Dec bits)  anything else -- the window passes RA = 0/360, is wider than one cell (polar rows),
+//                          or touches both neighbouring zones: such rows take the general per-lane path
 constexpr int kKeyFlagShift = 28;
 constexpr uint32_t kKeyMask = (1u << kKeyFlagShift) - 1u;
-constexpr uint32_t kKeyExtLo = 1u << 28, kKeyExtHi = 1u << 29, kKeySlow = 1u << 30;
+constexpr uint32_t kKeyExtLo = 1u << 28, kKeyExtHi = 1u << 29, kKeyDecLo = 1u << 30, kKeyDecHi = 1u << 31;
+constexpr uint32_t kKeyGeneral = kKeyDecLo | kKeyDecHi;
 
 // ---- grid as the kernels see it (passed by value) ----------------------------------------
 struct GridView {
@@ -46,10 +48,16 @@ struct GridView {
 };
 
 // tile of the cell-sorted catalogue: rows [first, first + count) all lie in `zone`, in its cells k_first..k_last
+// flags: which neighbours some row of the tile reaches (OR of the rows' window flags)
+constexpr uint32_t kTileDecLo = 1u, kTileDecHi = 2u, kTileGeneral = 4u;
+// besides its rows the descriptor carries what a match needs to know about the tile's zone and its neighbours, so that
+// no look-up depends on another one: RA cells n of the zone (and 1 / n), first cell key cb, cells of the zones below / above
 struct TileDesc {
-    uint32_t first, count, zone, k_first, k_last, pad0, pad1, pad2;
+    uint32_t first, count, zone, k_first;
+    uint32_t k_last, flags, n, cb;
+    uint32_t n_lo, n_hi; double inv_n;          // n_lo / n_hi = 0: no such zone
 };
-static_assert(sizeof(TileDesc) == 32, "TileDesc is read as two 16-byte words");
+static_assert(sizeof(TileDesc) == 48, "TileDesc is read as three 16-byte words");
 
 struct IndexView {
     const double* x; const double* y; const double* z;   // [n] unit vectors, cell order
@@ -95,7 +103,7 @@ void launch_gather(const Rec* rec, const uint32_t* perm, uint32_t n, double* x, 
 size_t cell_big_cap(size_t n_cells);
 void launch_cell_table(const uint32_t* sorted_keys, uint32_t key_mask, uint32_t n, uint32_t n_cells, uint32_t* cell_start,
                        uint32_t* d_big, cudaStream_t s);
-void launch_tiles(const uint32_t* cell_start, const uint32_t* cell_base, uint32_t n_zones, const uint32_t* sorted_keys,
+void launch_tiles(const uint32_t* cell_start, const uint32_t* cell_base, const int32_t* n_ra, uint32_t n_zones, const uint32_t* sorted_keys,
                   uint32_t key_mask, uint32_t tile_cap, uint32_t* d_tile_first, TileDesc* tiles, uint32_t* d_n_tiles, cudaStream_t s);
 
 size_t match_temp_bytes(const IndexView& A, const IndexView& B);

@@ -32,12 +32,10 @@
 
 #include <algorithm>
 
-#include "hlc2_grid.cuh"
+#include "hlc2_match_common.cuh"
 
 namespace hlc2 {
 
-constexpr int kCW = kTile / 32;              // consumer warps (one lane per A row of the tile)
-constexpr int kMatchThreads = kTile + 32;    // + the producer warp
 #ifndef HLC2_STAGES
 #define HLC2_STAGES 2
 #endif
@@ -47,9 +45,6 @@ constexpr int kMatchThreads = kTile + 32;    // + the producer warp
 #ifndef HLC2_CSCAP
 #define HLC2_CSCAP 1024
 #endif
-#ifndef HLC2_QCAP
-#define HLC2_QCAP 64
-#endif
 #ifndef HLC2_CTAS
 #define HLC2_CTAS 6
 #endif
@@ -57,17 +52,8 @@ constexpr int kStages = HLC2_STAGES;
 constexpr int kSegs = 3;                     // window pieces per job
 constexpr int kBCap = HLC2_BCAP;             // staged B rows per job, all pieces, after 16-byte alignment
 constexpr int kCsCap = HLC2_CSCAP;           // staged cell_start entries per job, after alignment
-constexpr int kQCap = HLC2_QCAP;             // rows in a warp's hit queue
-constexpr int kQFlush = kQCap - 32;          // flushed as soon as this many are queued (at most kQFlush - 1 + 32 are ever held)
 constexpr int kAPad = kTile + 2;             // A tile rows after alignment to 16 bytes
 constexpr int kMaxZones = 8;                 // tiles whose window spans more zones of B's grid take the general path
-constexpr double kRad2Arcsec = 206264.80624709636;   // 648000 / pi
-constexpr unsigned kFull = 0xffffffffu;
-
-// padding of the fp32 position estimate (degrees); derivation in DESIGN.md section 5 (~3x the worst case)
-constexpr double kEpsRaDeg = 2.5e-4;
-constexpr double kEpsDecDeg = 1.5e-4;
-constexpr double kTinyDeg = 1e-9;            // fp64 slop on cell / zone edges in the planner
 
 // job flags (bits 0-3: number of pieces)
 constexpr uint32_t kJobDirect = 1u << 8;     // general per-lane path from global memory
@@ -76,8 +62,6 @@ constexpr uint32_t kJobWrap = 1u << 10;      // window touches u = 0 / 360: rows
 constexpr uint32_t kJobFirst = 1u << 11;     // first / last job of its A tile (nearest mode carries the best across jobs)
 constexpr uint32_t kJobLast = 1u << 12;
 constexpr uint32_t kJobEnd = 1u << 13;       // producer -> consumers: no more work
-constexpr uint32_t kJobSame = 1u << 14;      // A and B share one grid: rows find their cells from their own key + window flags
-constexpr int kDqCap = 64;                   // rows a consumer warp holds back for the general path (drained 32 at a time)
 
 // 128-byte job record (32 words).  jobs[t] is the first job of A tile t; further jobs of a tile (windows that do
 // not fit one stage: the paper's calculation blocks, L253-257, cut to fit shared memory) are chained by `next`.
@@ -86,77 +70,23 @@ struct JobSeg { int32_t zone, k_lo; uint32_t nk, row_lo, n_rows; int32_t n_ra; u
 struct Job { uint32_t a_first, a_count, flags, next; JobSeg seg[kSegs]; uint32_t pad[4]; };
 static_assert(sizeof(JobSeg) == 32 && sizeof(Job) == 128, "the producer reads a job as 32 words");
 
-struct MatchArgs {
-    double thr2;          // 4 sin^2(r/2)
-    double pad_dec;       // r in degrees + kEpsDecDeg
-    double r_deg;
-    float sin_r_up;       // sin(r) * (1 + 1e-5)
-    int64_t* out_ida; int64_t* out_idb; double* out_sep;
-    unsigned long long capacity;
-    unsigned long long* count;
-    Job* jobs;            // [tile_cap] first jobs, then [pool_cap] chained jobs
-    uint32_t* pool_count;
-    uint32_t tile_cap, pool_cap;
-};
-
-struct SegDesc { double n_d; double centre; int32_t zone, k_lo, k_hi, cdelta; uint32_t rdelta, row_lo, row_hi; int32_t kbase; };
-struct StageDesc { uint32_t a_first, a_count, a_off, flags; int32_t nseg; uint32_t a_koff; SegDesc seg[kSegs]; };
+struct SegDesc { double n_d; double centre; int32_t zone, k_lo, k_hi, cdelta; uint32_t rdelta, row_lo, row_hi; int32_t pad; };
+struct StageDesc { uint32_t a_first, a_count, a_off, flags; int32_t nseg; uint32_t pad; SegDesc seg[kSegs]; };
 
 struct __align__(16) Stage {
     double ax[kAPad], ay[kAPad], az[kAPad];
-    float2 apos[kAPad];                                     // same-grid jobs: the rows' flagged cell keys (uint32) instead
+    float2 apos[kAPad];
     double bx[kBCap + 2], by[kBCap + 2], bz[kBCap + 2];     // slot kBCap: a point no chord test can reach
     uint32_t cs[kCsCap];
     StageDesc d;
 };
-// ids are looked up when a queue is flushed (32 rows at a time, overlapped with the atomic), so neither catalogue's
-// id column is staged: the queue holds the global A and B row numbers
-struct WarpQueue { uint32_t a[kQCap], b[kQCap]; double c2[kQCap]; };
 struct __align__(16) MatchSmem {
     Stage st[kStages];
     WarpQueue q[kCW];
-    uint32_t dq[kCW][kDqCap];
     unsigned long long full[kStages], empty[kStages];
 };
 static_assert((kAPad * 8) % 16 == 0 && (kBCap * 8) % 16 == 0 && (kCsCap * 4) % 16 == 0, "bulk copies need 16-byte pieces");
 static_assert(sizeof(Stage) % 16 == 0, "stages stay 16-byte aligned");
-
-// ---- mbarrier / bulk-copy primitives (sm_90+ PTX) ----------------------------------------------------
-__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(unsigned long long* b, unsigned count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(unsigned long long* b) {
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* b, unsigned bytes) {
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
-}
-// try_wait suspends the thread in hardware until the phase completes or the time hint (ns) runs out, so a long
-// hint costs no wake-up latency and spares the issue slots a polling loop would burn
-__device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity) {
-    const uint32_t a = smem_u32(b);
-    unsigned done;
-    do {
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n selp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(done) : "r"(a), "r"(parity), "r"(0x4000u) : "memory");
-    } while (!done);
-}
-// global -> shared bulk copy, completion counted in bytes on an mbarrier; 16-byte aligned src, dst and size
-__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* b) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(b)) : "memory");
-}
-
-// sep = 2 asin(chord / 2) in arcsec.  Below 2^-10 rad (403 arcsec) the series h + h^3/6 + 3 h^5/40 is exact to
-// 4e-20 relative; above it the library asin.
-__device__ __forceinline__ double sep_from_chord2(double c2) {
-    const double h = 0.5 * sqrt(c2);
-    double a;
-    if (h < 0.0009765625) { const double t = h * h; a = fma(h * t, fma(t, 0.075, 1.0 / 6.0), h); }
-    else a = asin(fmin(1.0, h));
-    return a * (2.0 * kRad2Arcsec);
-}
 
 // ------------------------------------------------------------------------------------------------------
 // k_plan: the jobs of every A tile
@@ -226,7 +156,6 @@ __device__ __noinline__ void plan_piece(PlanState& st, const MatchArgs& p, const
     }
 }
 
-template <bool SAME>
 __global__ void __launch_bounds__(128)
 k_plan(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B, const __grid_constant__ MatchArgs p) {
     const uint32_t nt = __ldg(A.n_tiles);
@@ -234,7 +163,7 @@ k_plan(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B,
     const GridView& gb = B.g;
     for (uint32_t t = blockIdx.x * 128 + threadIdx.x; t < nt; t += gridDim.x * 128) {
         const uint4 t0 = __ldg(reinterpret_cast<const uint4*>(A.tiles + t));        // first, count, zone, k_first
-        const uint4 t1 = __ldg(reinterpret_cast<const uint4*>(A.tiles + t) + 1);    // k_last
+        const uint4 t1 = __ldg(reinterpret_cast<const uint4*>(A.tiles + t) + 1);    // k_last, flags, n, cb
         PlanState st;
 #pragma unroll
         for (int i = 0; i < 32; ++i) st.w[i] = 0;
@@ -249,17 +178,7 @@ k_plan(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B,
         const bool empty = qhi < gb.dec_min || qlo > gb.dec_max || t0.y == 0;
         bool direct = false;
         uint32_t common = 0;
-        if (SAME) {
-            // one grid for both catalogues: the rows of the tile sit in cells k_first..k_last of zone za, their window
-            // flags (index build) say which of them reach one cell further, and rows whose window leaves the zone are
-            // handled by the general path; so the tile's staged window is cells k_first-1 .. k_last+1 of the same zone
-            common = kJobSame;
-            if (t0.y != 0) {
-                const int n = __ldg(gb.n_ra + za);
-                plan_piece(st, p, B.cell_start, common, za, n, __ldg(gb.cell_base + za), max((int)t0.w - 1, 0), min((int)t1.x + 1, n - 1), 0.0f);
-                if (st.overflow) direct = true;
-            }
-        } else if (!empty) {
+        if (!empty) {
             const int zb0 = zone_of(gb, qlo), zb1 = zone_of(gb, qhi);
             if (zb1 - zb0 + 1 > kMaxZones) direct = true;
             const double cw = ga.span / (double)__ldg(ga.n_ra + za);
@@ -313,105 +232,6 @@ k_plan(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B,
         } else {
             plan_close(st, p, common, true);        // a tile without pieces ends up as one empty job
         }
-    }
-}
-
-// ------------------------------------------------------------------------------------------------------
-// the general per-lane path (DIRECT tiles): any number of zones, RA wrap, polar ring, window partly outside
-// B's box.  Reads B through global memory / L2.
-// ------------------------------------------------------------------------------------------------------
-struct Best { double c2; uint32_t row; bool has; };      // row: global B row
-
-// one row straight to the output; lanes that arrive together share one global atomic
-__device__ __forceinline__ void emit_direct(const IndexView& A, const IndexView& B, const MatchArgs& p, uint32_t a_row, uint32_t b_row, double c2) {
-    const unsigned m = __activemask();
-    const int lane = threadIdx.x & 31, leader = __ffs(m) - 1;
-    unsigned long long base = 0;
-    if (lane == leader) base = atomicAdd(p.count, (unsigned long long)__popc(m));
-    base = __shfl_sync(m, base, leader);
-    const unsigned long long o = base + __popc(m & ((1u << lane) - 1u));
-    if (o < p.capacity) { p.out_ida[o] = __ldg(A.id + a_row); p.out_idb[o] = __ldg(B.id + b_row); p.out_sep[o] = sep_from_chord2(c2); }
-}
-
-template <int MODE>
-__device__ __forceinline__ void scan_global(const IndexView& A, const IndexView& B, const MatchArgs& p, uint32_t a_row,
-                                            double ax, double ay, double az, uint32_t j0, uint32_t j1, Best& h) {
-    for (uint32_t j = j0; j < j1; ++j) {
-        const double dx = ax - __ldg(B.x + j), dy = ay - __ldg(B.y + j), dz = az - __ldg(B.z + j);
-        const double c2 = fma(dx, dx, fma(dy, dy, dz * dz));
-        if (c2 <= p.thr2) {
-            if (MODE == HLC2_ALL_PAIRS) emit_direct(A, B, p, a_row, j, c2);
-            else if (!h.has || c2 < h.c2 || (c2 == h.c2 && __ldg(B.id + j) < __ldg(B.id + h.row))) { h.has = true; h.row = j; h.c2 = c2; }
-        }
-    }
-}
-
-template <int MODE>
-__device__ __noinline__ void scan_general(const IndexView& A, const IndexView& B, const MatchArgs& p, uint32_t a_row,
-                                          double ax, double ay, double az, float2 pf, Best& h) {
-    const GridView& g = B.g;
-    const double dlo = (double)pf.y - p.pad_dec, dhi = (double)pf.y + p.pad_dec;
-    if (!(dhi >= g.dec_min && dlo <= g.dec_max)) return;          // also rows with a bad coordinate (NaN vector)
-    const float fx = (float)ax, fy = (float)ay;
-    const float s = p.sin_r_up * rsqrtf(fx * fx + fy * fy);               // sin(dRA_max) = sin r / cos dec
-    const bool ring = !(s < 0.25f);
-    const double w = ring ? 360.0 : (double)(s * (1.011f * 57.29577951f)) + kEpsRaDeg;   // asin(s) <= 1.011 s below 0.25
-    const double u = box_u(g, (double)pf.x);
-    const double ulo = u - w, uhi = u + w;
-    const int z0 = zone_of(g, dlo), z1 = zone_of(g, dhi);
-    for (int z = z0; z <= z1; ++z) {
-        const int n = __ldg(g.n_ra + z);
-        const uint32_t base = __ldg(g.cell_base + z);
-        int k0 = 0, k1 = n - 1, k2 = 0, k3 = -1;      // [k0,k1] and optional [k2,k3]
-        if (!(ring || w >= 180.0)) {
-            const bool va = ulo <= g.span;
-            k0 = cell_of_u(g, fmax(ulo, 0.0), n); k1 = cell_of_u(g, fmin(uhi, g.span), n);
-            bool vx = false;
-            if (ulo < 0.0) { if (ulo + 360.0 <= g.span) { vx = true; k2 = cell_of_u(g, ulo + 360.0, n); k3 = n - 1; } }
-            else if (uhi >= 360.0) { vx = true; k2 = 0; k3 = cell_of_u(g, fmin(uhi - 360.0, g.span), n); }
-            if (va && vx && !(k3 < k0 || k2 > k1)) { k0 = 0; k1 = n - 1; vx = false; }
-            if (!va) { if (!vx) continue; k0 = k2; k1 = k3; vx = false; }
-            if (!vx) k3 = k2 - 1;
-        }
-        scan_global<MODE>(A, B, p, a_row, ax, ay, az, __ldg(B.cell_start + base + k0), __ldg(B.cell_start + base + k1 + 1), h);
-        if (k3 >= k2)
-            scan_global<MODE>(A, B, p, a_row, ax, ay, az, __ldg(B.cell_start + base + k2), __ldg(B.cell_start + base + k3 + 1), h);
-    }
-}
-
-// ------------------------------------------------------------------------------------------------------
-// hit queue of one consumer warp
-// ------------------------------------------------------------------------------------------------------
-// write queue rows [first, first + cnt) to the output: one global atomic, coalesced stores
-__device__ __forceinline__ void flush_rows(const IndexView& A, const IndexView& B, const MatchArgs& p, const WarpQueue& q,
-                                           unsigned first, unsigned cnt, int lane) {
-    unsigned long long base = 0;
-    if (lane == 0) base = atomicAdd(p.count, (unsigned long long)cnt);
-    base = __shfl_sync(kFull, base, 0);
-    for (unsigned k = lane; k < cnt; k += 32) {
-        const unsigned long long o = base + k;
-        if (o < p.capacity) {
-            p.out_ida[o] = __ldg(A.id + q.a[first + k]); p.out_idb[o] = __ldg(B.id + q.b[first + k]);
-            p.out_sep[o] = sep_from_chord2(q.c2[first + k]);
-        }
-    }
-}
-
-// append the lanes with `hit`; flush the top kQFlush rows once that many are queued.  qn is warp-uniform.
-__device__ __forceinline__ void push_hits(const IndexView& A, const IndexView& B, const MatchArgs& p, WarpQueue& q, unsigned& qn,
-                                          bool hit, uint32_t a_row, uint32_t b_row, double c2, int lane) {
-    const unsigned m = __ballot_sync(kFull, hit);
-    if (m == 0) return;
-    if (hit) {
-        const unsigned k = qn + __popc(m & ((1u << lane) - 1u));
-        q.a[k] = a_row; q.b[k] = b_row; q.c2[k] = c2;
-    }
-    qn += __popc(m);
-    if (qn >= (unsigned)kQFlush) {
-        __syncwarp();
-        qn -= kQFlush;
-        flush_rows(A, B, p, q, qn, kQFlush, lane);
-        __syncwarp();
     }
 }
 
@@ -492,23 +312,10 @@ __device__ __forceinline__ void seg_ranges(const IndexView& A, const IndexView& 
     }
 }
 
-// rows of same-grid tiles whose window leaves their own zone (window flag kKeySlow): the general per-lane path, one
-// full warp of them at a time, from global memory (their tile was just staged, so the lines are in L2)
-template <int MODE>
-__device__ __noinline__ void drain_deferred(const IndexView& A, const IndexView& B, const MatchArgs& p, WarpQueue& q, unsigned& qn,
-                                            const uint32_t* dq, unsigned cnt, int lane) {
-    const bool act = (unsigned)lane < cnt;
-    const uint32_t a_row = act ? dq[lane] : 0u;
-    Best h; h.has = false; h.c2 = 0.0; h.row = 0;
-    if (act) scan_general<MODE>(A, B, p, a_row, __ldg(A.x + a_row), __ldg(A.y + a_row), __ldg(A.z + a_row), __ldg(A.pos + a_row), h);
-    __syncwarp();
-    if (MODE == HLC2_NEAREST) push_hits(A, B, p, q, qn, act && h.has, a_row, h.row, h.c2, lane);
-}
-
 // ------------------------------------------------------------------------------------------------------
 // k_match
 // ------------------------------------------------------------------------------------------------------
-template <int MODE, bool SAME>
+template <int MODE>
 __global__ void __launch_bounds__(kMatchThreads, HLC2_CTAS)
 k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B, const __grid_constant__ MatchArgs p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -568,21 +375,18 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
                 rtot += a; ctot += c;
             }
             const bool any = nseg != 0 || (flags & kJobDirect);
-            const bool same = SAME && (flags & kJobSame) != 0;
             const uint32_t a_al = a_first & ~1u;
             const uint32_t a_ld = any ? (((a_first + a_count + 1u) & ~1u) - a_al) : 0u;
-            const uint32_t k_al = a_first & ~3u;                                   // same-grid jobs stage 4-byte keys, not 8-byte pos
-            const uint32_t k_ld = any && same ? (((a_first + a_count + 3u) & ~3u) - k_al) : 0u;
-            const uint32_t bytes = a_ld * (same ? 24u : 32u) + k_ld * 4u + rtot * 24u + ctot * 4u;
+            const uint32_t bytes = a_ld * 32u + rtot * 24u + ctot * 4u;
 
             mbar_wait(&sm.empty[s], ph ^ 1u);
-            if (lane == 0) { st.d.a_first = a_first; st.d.a_count = a_count; st.d.a_off = a_first - a_al; st.d.flags = flags; st.d.nseg = nseg; st.d.a_koff = a_first - k_al; }
+            if (lane == 0) { st.d.a_first = a_first; st.d.a_count = a_count; st.d.a_off = a_first - a_al; st.d.flags = flags; st.d.nseg = nseg; }
             if (segact) {
                 SegDesc& e = st.d.seg[lane];
                 e.n_d = (double)(int32_t)n_ra; e.centre = (double)__uint_as_float(ctr);
                 e.zone = (int32_t)zone; e.k_lo = (int32_t)k_lo; e.k_hi = (int32_t)(k_lo + nk) - 1;
                 e.cdelta = (int32_t)((cs_lo - k_lo) - cs_al + coff); e.rdelta = roff - row_al;
-                e.row_lo = row_lo; e.row_hi = row_lo + nr; e.kbase = (int32_t)(cs_lo - k_lo);
+                e.row_lo = row_lo; e.row_hi = row_lo + nr;
             }
             __syncwarp();
             if (lane == 0) { if (bytes) mbar_arrive_expect_tx(&sm.full[s], bytes); else mbar_arrive(&sm.full[s]); }
@@ -595,9 +399,9 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
             if (a_ld && lane >= 8 && lane < 12) {
                 const int k = lane - 8;
                 const void* src = k == 0 ? (const void*)(A.x + a_al) : k == 1 ? (const void*)(A.y + a_al) : k == 2 ? (const void*)(A.z + a_al)
-                                : same ? (const void*)(A.key + k_al) : (const void*)(A.pos + a_al);
+                                : (const void*)(A.pos + a_al);
                 void* dst = k == 0 ? (void*)st.ax : k == 1 ? (void*)st.ay : k == 2 ? (void*)st.az : (void*)st.apos;
-                bulk_g2s(dst, src, k == 3 && same ? k_ld * 4u : a_ld * 8u, &sm.full[s]);
+                bulk_g2s(dst, src, a_ld * 8u, &sm.full[s]);
             }
             wcur = wnext; have = nhave;
         }
@@ -611,8 +415,7 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
     // ---------------- consumer warps: one lane per A row of the tile ----------------
     const GridView& g = B.g;
     WarpQueue& q = sm.q[warp];
-    uint32_t* dq = sm.dq[warp];
-    unsigned qn = 0, dn = 0;
+    unsigned qn = 0;
     Best best; best.has = false; best.c2 = 0.0; best.row = 0;
     for (uint32_t it = 0;; ++it) {
         const int s = (int)(it % kStages);
@@ -627,38 +430,14 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
             const bool act = threadIdx.x < a_count;
             if (MODE == HLC2_NEAREST && (flags & kJobFirst)) best.has = false;
             const uint32_t a_row = d.a_first + threadIdx.x;
-            if (SAME && (flags & kJobSame)) {
-                const unsigned ra = act ? threadIdx.x + d.a_off : d.a_off;
-                const double ax = st.ax[ra], ay = st.ay[ra], az = st.az[ra];
-                const uint32_t kf = reinterpret_cast<const uint32_t*>(st.apos)[(act ? threadIdx.x : 0u) + d.a_koff];
-                const bool slow = (kf & kKeySlow) != 0;
-                if (flags & kJobFirst) {            // rows whose window leaves their zone: held back for the general path, once per tile
-                    const unsigned m = __ballot_sync(kFull, act && slow);
-                    if (m) {
-                        if (act && slow) dq[dn + __popc(m & ((1u << lane) - 1u))] = a_row;
-                        dn += __popc(m);
-                    }
-                }
-                const int klo = (int)(kf & kKeyMask) - (int)((kf >> kKeyFlagShift) & 1u);
-                const int khi = (int)(kf & kKeyMask) + (int)((kf >> (kKeyFlagShift + 1)) & 1u);
-                for (int sg = 0; sg < nseg; ++sg) {
-                    const SegDesc& e = d.seg[sg];
-                    const int k0 = max(klo - e.kbase, e.k_lo), k1 = min(khi - e.kbase, e.k_hi);     // zone-local cells, clipped to the piece
-                    unsigned q0 = 0, q1 = 0;
-                    if (act && !slow && k0 <= k1) {
-                        q0 = min(max(st.cs[k0 + e.cdelta], e.row_lo), e.row_hi) + e.rdelta;
-                        q1 = min(max(st.cs[k1 + 1 + e.cdelta], e.row_lo), e.row_hi) + e.rdelta;
-                    }
-                    scan_staged<MODE>(A, B, st, p, q, qn, a_row, ax, ay, az, q0, q1, e.rdelta, best, lane);
-                }
-            } else if (nseg != 0 || (flags & kJobDirect)) {
+            if (nseg != 0 || (flags & kJobDirect)) {
                 const unsigned ra = act ? threadIdx.x + d.a_off : d.a_off;
                 const double ax = st.ax[ra], ay = st.ay[ra], az = st.az[ra];
                 const float2 pf = st.apos[ra];
                 if (flags & kJobDirect) {
                     if (act) scan_general<MODE>(A, B, p, a_row, ax, ay, az, pf, best);
                     __syncwarp();
-                } else if (!SAME) {
+                } else {
                     const double dlo = (double)pf.y - p.pad_dec, dhi = (double)pf.y + p.pad_dec;
                     const int zlo = zone_of(g, dlo), zhi = zone_of(g, dhi);
                     const float fx = (float)ax, fy = (float)ay;
@@ -679,24 +458,17 @@ k_match(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm.empty[s]);
-        if (SAME && dn >= 32u) {                    // a full warp of held-back rows: general path, off the stage
-            drain_deferred<MODE>(A, B, p, q, qn, dq, 32u, lane);
-            const uint32_t v = lane + 32u < dn ? dq[lane + 32u] : 0u;
-            __syncwarp();
-            if (lane + 32u < dn) dq[lane] = v;
-            dn -= 32u;
-            __syncwarp();
-        }
     }
     __syncwarp();
-    if (SAME && dn) drain_deferred<MODE>(A, B, p, q, qn, dq, dn, lane);
     if (qn) flush_rows(A, B, p, q, 0, qn, lane);
 }
 
 static inline size_t pool_cap_of(size_t tile_cap) { return 3 * tile_cap + 4096; }
 
 size_t match_temp_for_tiles(size_t tile_cap) { return (tile_cap + pool_cap_of(tile_cap)) * sizeof(Job) + 256; }
-size_t match_temp_bytes(const IndexView& A, const IndexView& B) { return match_temp_for_tiles(std::max(A.tile_cap, B.tile_cap)); }
+size_t match_temp_bytes(const IndexView& A, const IndexView& B) {
+    return std::max(match_temp_for_tiles(std::max(A.tile_cap, B.tile_cap)), match_same_temp_bytes(A));
+}
 
 void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_arcsec, int mode,
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
@@ -711,7 +483,8 @@ void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_ar
     // work (window, cell look-ups) is paid by the catalogue whose rows drive the lanes, while staging grows with the
     // scanned rows per driving row; measured on config 3 (ratio 2) the two directions tie, so the roles are
     // exchanged only when B is much the smaller catalogue.
-    const bool swap = mode == HLC2_ALL_PAIRS && (size_t)B_in.n * 3 < (size_t)A_in.n;
+    const bool same = (match_flags & kMatchSameGrid) != 0;
+    const bool swap = !same && mode == HLC2_ALL_PAIRS && (size_t)B_in.n * 3 < (size_t)A_in.n;
     const IndexView& A = swap ? B_in : A_in;
     const IndexView& B = swap ? A_in : B_in;
     if (swap) std::swap(out_ida, out_idb);
@@ -723,17 +496,20 @@ void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_ar
     p.pad_dec = p.r_deg + kEpsDecDeg;
     p.sin_r_up = (float)((double)sinl(r_rad) * (1.0 + 1e-5));
     p.out_ida = out_ida; p.out_idb = out_idb; p.out_sep = out_sep; p.capacity = capacity; p.count = d_count;
+    p.jobs = nullptr; p.pool_count = nullptr; p.tile_cap = 0; p.pool_cap = 0;
+    if (same) {         // both indices on one grid: no planner, no job records (hlc2_match_same.cu)
+        launch_match_same(A, B, p, mode, d_temp, s, ev_start, ev_stop);
+        return;
+    }
     const size_t tiles = A.tile_cap;
     // scratch: 256-byte header (pool counter), then the tiles' first jobs, then the pool of chained jobs
     p.pool_count = reinterpret_cast<uint32_t*>(d_temp);
     p.jobs = reinterpret_cast<Job*>(reinterpret_cast<char*>(d_temp) + 256);
     p.tile_cap = (uint32_t)tiles; p.pool_cap = (uint32_t)pool_cap_of(tiles);
     cudaMemsetAsync(p.pool_count, 0, sizeof(uint32_t), s);
-    const bool same = (match_flags & kMatchSameGrid) != 0;
-    const int m = (mode == HLC2_NEAREST ? 1 : 0) + (same ? 2 : 0);
-    const void* kern = m == 0 ? (const void*)k_match<HLC2_ALL_PAIRS, false> : m == 1 ? (const void*)k_match<HLC2_NEAREST, false>
-                     : m == 2 ? (const void*)k_match<HLC2_ALL_PAIRS, true> : (const void*)k_match<HLC2_NEAREST, true>;
-    static int per_sm_dev[kMaxDevices][4] = {};        // resident CTAs per SM; the smem opt-in is per device
+    const int m = mode == HLC2_NEAREST ? 1 : 0;
+    const void* kern = m == 0 ? (const void*)k_match<HLC2_ALL_PAIRS> : (const void*)k_match<HLC2_NEAREST>;
+    static int per_sm_dev[kMaxDevices][2] = {};        // resident CTAs per SM; the smem opt-in is per device
     int* per_sm = per_sm_dev[current_device()];
     const size_t smem = sizeof(MatchSmem);
     if (!per_sm[m]) {
@@ -743,8 +519,7 @@ void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_ar
         per_sm[m] = v > 0 ? v : 1;
     }
     const unsigned pblocks = (unsigned)std::min<size_t>((tiles + 127) / 128, (size_t)sm_count() * 8);
-    if (same) k_plan<true><<<pblocks, 128, 0, s>>>(A, B, p);
-    else                              k_plan<false><<<pblocks, 128, 0, s>>>(A, B, p);
+    k_plan<<<pblocks, 128, 0, s>>>(A, B, p);
     count_launch();
     // persistent grid: SM count x resident CTAs, never more CTAs than tiles
     const unsigned blocks = (unsigned)std::max<size_t>(1, std::min<size_t>(tiles, (size_t)sm_count() * per_sm[m]));

@@ -143,7 +143,7 @@ def test_seam_tile_next_to_one_cell_polar_zone(P, mode):
     that zone edge within the RA window of the seam reach the polar cell through both images of their window; every
     pair must be reported exactly once (tests/parity.py asserts uniqueness)."""
     rng = np.random.default_rng(160)
-    o = P.make_opts(3.0, cell_arcsec=160.0, full_sky=True)
+    o = P.make_opts(3.0, cell_arcsec=160.0, full_sky=True, zone_aspect=1)       # square cells: zones 160 arcsec high
     parts_ra, parts_dec = [], []
     for sign in (1.0, -1.0):
         edge = 90.0 - 160.0 / 3600.0

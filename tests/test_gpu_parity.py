@@ -63,7 +63,7 @@ def test_index_invariants(P, cfg, scale):
     key = arr["cell_key"].cpu().numpy().view(np.uint32).astype(np.int64)
     flags = key >> 28                                  # window flags ride in the top bits (include/hlc2.h, HLC2_KEY_MASK)
     key = key & P.HLC2_KEY_MASK
-    assert flags.max() <= 4 and ((flags & 4 == 0) | (flags == 4)).all()
+    assert flags.max() <= 15
     cs = arr["cell_start"].cpu().numpy().view(np.uint32).astype(np.int64)
     assert (np.diff(key) >= 0).all() and key.max() < nc
     assert cs[0] == 0 and cs[-1] == n and (np.diff(cs) >= 0).all()
@@ -78,6 +78,17 @@ def test_index_invariants(P, cfg, scale):
     assert np.abs(z - np.sin(d)).max() < 2e-15
     g = P.hlc2_grid_describe(idx)
     assert g["n_cells"] == nc and g["n_ra"].sum() == nc and g["cell_arcsec"] >= w.radius_arcsec
+    # window flags (bits 30 / 31: the window reaches the zone below / above; both: general path): a row within r_max of
+    # a zone edge must carry that edge's flag, a row further than r_max (+ slop) from both edges must carry neither
+    dec_s = np.rad2deg(np.arcsin(np.clip(z, -1.0, 1.0)))
+    zone = np.clip(np.floor((dec_s - g["dec_lo"]) / g["zone_h"]).astype(np.int64), 0, g["n_zones"] - 1)
+    d_lo = dec_s - (g["dec_lo"] + zone * g["zone_h"]); d_hi = (g["dec_lo"] + (zone + 1) * g["zone_h"]) - dec_s
+    r_deg = w.radius_arcsec / 3600.0
+    general = (flags >> 2) == 3
+    need_lo = (d_lo < r_deg - 1e-7) & (zone > 0); need_hi = (d_hi < r_deg - 1e-7) & (zone < g["n_zones"] - 1)
+    assert (((flags >> 2) & 1)[need_lo] == 1).all() and (((flags >> 3) & 1)[need_hi] == 1).all()
+    far = (d_lo > r_deg + 1e-6) & (d_hi > r_deg + 1e-6) & ~general
+    assert ((flags >> 2)[far] == 0).all()
     # occupancy near the target (1 source per cell over the occupied box)
     assert 0.2 < n / nc < 5.0
 
@@ -161,7 +172,10 @@ def test_poles_seam_duplicates_micro(P, radius, mode):
     A, B = _tiny()
     for kw in ({}, {"full_sky": True}, {"cell_arcsec": radius}, {"cell_arcsec": 20000.0}):
         check(P, A, B, radius, mode, engine=oracle.ENGINE_BRUTE_LD, **kw)
-        check(P, A, B, radius, mode, engine=oracle.ENGINE_BRUTE_LD, same_grid=True, **kw)
+        try:
+            check(P, A, B, radius, mode, engine=oracle.ENGINE_BRUTE_LD, same_grid=True, **kw)
+        except P.Hlc2Error as e:        # B's few hundred sources leave RA gaps: its box may not hold all of A
+            assert e.status == P.HLC2_ERR_GRID_MISMATCH and not kw.get("full_sky")
 
 
 def test_patch_across_ra_seam_and_on_pole(P):
