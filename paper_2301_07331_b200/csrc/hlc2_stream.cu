@@ -13,6 +13,8 @@
 // Every A source lives in exactly one band and sees one B window, so nearest mode needs no merge step.
 // Device memory is the caller's arena (hlc2_stream_sizes): 2 raw A slots, 4 raw B slots, the window's raw
 // columns, two index buffers, build / match scratch and 2 output slots.
+#include <string.h>
+
 #include <algorithm>
 
 #include "hlc2_internal.cuh"
@@ -65,13 +67,13 @@ static int stream_arena(int64_t max_a, int64_t max_b, const hlc2_opts* opts, int
     size_t ia = 0, ta = 0, ib = 0, tb = 0;
     int rc = hlc2_index_sizes(max_a, opts, &ia, &ta); if (rc != HLC2_OK) return rc;
     rc = hlc2_index_sizes((int64_t)L->win_cap, opts, &ib, &tb); if (rc != HLC2_OK) return rc;
-    L->ib_a = ia; L->ib_b = ib;
+    L->ib_a = std::max(ia, ib); L->ib_b = ib;      // A bands are filed on the window's grid: its cell table can be the larger one
     L->tb = std::max(std::max(ta, tb), match_temp_bound(max_a, opts));
     size_t off = 0;
     for (int i = 0; i < 2; ++i) { L->raw_a[i] = off; off += up256((size_t)max_a * 8) * 3; }
     for (int i = 0; i < 4; ++i) { L->raw_b[i] = off; off += up256((size_t)max_b * 8) * 3; }
     L->win = off; off += up256(L->win_cap * 8) * 3;
-    L->idx_a = off; off += up256(ia);
+    L->idx_a = off; off += up256(L->ib_a);
     L->idx_b = off; off += up256(ib);
     L->temp = off; off += up256(L->tb);
     for (int i = 0; i < 2; ++i) { L->out[i] = off; off += up256((size_t)max_out * 8) * 3; }
@@ -249,8 +251,19 @@ int hlc2_stream_crossmatch(const double* h_a_ra, const double* h_a_dec, const in
             k_iota_ids<<<(unsigned)std::min<size_t>((na + 255) / 256, (size_t)sms * 8), 256, 0, R.comp>>>((long long*)(ak + 2 * sa), (long long)h_a_off[k], (uint32_t)na);
             count_launch();
         }
-        RC(hlc2_build_index((const double*)ak, (const double*)(ak + sa), (const int64_t*)(ak + 2 * sa), (int64_t)na, opts,
-                            base + L.idx_a, L.ib_a, base + L.temp, L.tb, R.comp, &ga.h));
+        // A band k is filed on the window's grid (opts.grid_like), so that the match takes its same-grid path; a band
+        // that does not fit inside the window's RA box (a patch of A with no B nearby) gets a grid of its own
+        {
+            hlc2_opts oa;
+            if (opts) oa = *opts; else { memset(&oa, 0, sizeof oa); oa.r_max_arcsec = 1.0; }
+            oa.grid_like = gb.h;
+            int rc_a = hlc2_build_index((const double*)ak, (const double*)(ak + sa), (const int64_t*)(ak + 2 * sa), (int64_t)na, &oa,
+                                        base + L.idx_a, L.ib_a, base + L.temp, L.tb, R.comp, &ga.h);
+            if (rc_a == HLC2_ERR_GRID_MISMATCH || rc_a == HLC2_ERR_BUFFER_TOO_SMALL)
+                rc_a = hlc2_build_index((const double*)ak, (const double*)(ak + sa), (const int64_t*)(ak + 2 * sa), (int64_t)na, opts,
+                                        base + L.idx_a, L.ib_a, base + L.temp, L.tb, R.comp, &ga.h);
+            RC(rc_a);
+        }
         char* ok_ = base + L.out[k & 1];
         CK(cudaStreamWaitEvent(R.comp, R.free_out[k & 1], 0));      // band k-2's rows have left this slot
         RC(hlc2_crossmatch(ga.h, gb.h, radius_arcsec, mode, (int64_t*)ok_, (int64_t*)(ok_ + so), (double*)(ok_ + 2 * so),
