@@ -53,6 +53,12 @@ def _load():
                                           ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_int,
                                           ip, ctypes.POINTER(ip), ctypes.POINTER(ip), ctypes.POINTER(dp),
                                           ctypes.POINTER(ctypes.c_int)]
+        lib.hlc2_oracle_match_ext.restype = ctypes.c_int
+        lib.hlc2_oracle_match_ext.argtypes = [dp, dp, ip, ctypes.c_int64, dp, dp, ip, ctypes.c_int64,
+                                              ctypes.c_double, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                              dp, dp, ctypes.c_double, ctypes.c_int,
+                                              ip, ctypes.POINTER(ip), ctypes.POINTER(ip), ctypes.POINTER(dp),
+                                              ctypes.POINTER(ctypes.c_int)]
         lib.hlc2_oracle_free.restype = None
         lib.hlc2_oracle_free.argtypes = [ctypes.c_void_p]
         lib.hlc2_oracle_max_threads.restype = ctypes.c_int
@@ -81,13 +87,21 @@ def _f64(a):
     return np.ascontiguousarray(a, dtype=np.float64)
 
 
+SELF_NONE, SELF_PAIRS, SELF_PAIRS_AND_DIAGONAL, SELF_EXCLUDE_OWN = 0, 1, 2, 3
+
+
 def match(ra_a, dec_a, id_a, ra_b, dec_b, id_b, radius_arcsec, mode=ALL_PAIRS, engine=ENGINE_VOXEL,
-          threads=0):
+          threads=0, err_a=None, err_b=None, k_factor=3.0, self_mode=SELF_NONE):
     """Run the oracle.  Returns (idA, idB, sep_arcsec, threads_used), rows sorted by (idA, idB).
 
     ``id_a`` / ``id_b`` may be None (row numbers).  ``mode`` 0 = all pairs within the radius
     (inclusive), 1 = nearest B per A.  ``engine`` 0 = brute force all in long double,
     1 = brute force with fp64 pre-filter, 2 = voxel hash.
+
+    ``err_a`` / ``err_b`` (both or neither): per-record error radii in arcsec; the criterion becomes PAPER.md
+    Eq. (4) per pair, theta <= k_factor * sqrt(e1^2 + e2^2), capped by ``radius_arcsec``.  ``self_mode``: A and B
+    are one catalogue (pass the same arrays): 1 = every unordered pair {i, j}, i < j, once; 2 = those and (i, i);
+    3 = every ordered pair but j == i (for nearest: a source is not its own neighbour).
     """
     lib = _load()
     ra_a, dec_a, ra_b, dec_b = _f64(ra_a), _f64(dec_a), _f64(ra_b), _f64(dec_b)
@@ -105,11 +119,15 @@ def match(ra_a, dec_a, id_a, ra_b, dec_b, id_b, radius_arcsec, mode=ALL_PAIRS, e
     n = ctypes.c_int64(0)
     oa, ob, os_ = ip(), ip(), dp()
     used = ctypes.c_int(0)
-    rc = lib.hlc2_oracle_match(ra_a.ctypes.data_as(dp), dec_a.ctypes.data_as(dp), pa, ra_a.shape[0],
-                               ra_b.ctypes.data_as(dp), dec_b.ctypes.data_as(dp), pb, ra_b.shape[0],
-                               float(radius_arcsec), int(mode), int(engine), int(threads),
-                               ctypes.byref(n), ctypes.byref(oa), ctypes.byref(ob), ctypes.byref(os_),
-                               ctypes.byref(used))
+    ea = _f64(err_a) if err_a is not None else None
+    eb = _f64(err_b) if err_b is not None else None
+    rc = lib.hlc2_oracle_match_ext(ra_a.ctypes.data_as(dp), dec_a.ctypes.data_as(dp), pa, ra_a.shape[0],
+                                   ra_b.ctypes.data_as(dp), dec_b.ctypes.data_as(dp), pb, ra_b.shape[0],
+                                   float(radius_arcsec), int(mode), int(engine), int(threads),
+                                   ea.ctypes.data_as(dp) if ea is not None else dp(),
+                                   eb.ctypes.data_as(dp) if eb is not None else dp(), float(k_factor), int(self_mode),
+                                   ctypes.byref(n), ctypes.byref(oa), ctypes.byref(ob), ctypes.byref(os_),
+                                   ctypes.byref(used))
     if rc != 0:
         raise ValueError({-1: "bad coordinate (non-finite or |dec| > 90)", -2: "invalid argument",
                           -3: "out of memory"}.get(rc, f"oracle error {rc}"))

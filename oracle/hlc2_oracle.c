@@ -26,6 +26,12 @@
  *   - RA is any finite value, reduced modulo 360; |dec| <= 90 required.
  *   - (i,i) pairs are ordinary pairs; ids are opaque int64; output sorted by (idA,idB).
  *
+ * Extensions (hlc2_oracle_match_ext):
+ *   - per-record error radii: Eq. (4) (L68) as printed, theta <= k * sqrt(e1_i^2 + e2_j^2) with the paper's k = 3 a
+ *     parameter, evaluated in long double per pair; radius_arcsec is then a cap on the threshold (the search bound).
+ *   - self-match of one catalogue (the paper's D4 case, L286, L295): every unordered pair {i, j}, i < j by row, once;
+ *     optionally the n pairs (i, i) as well; nearest mode excludes a source from its own neighbours.
+ *
  * Engines:
  *   0  brute force, every (i,j) evaluated in long double          (tiny inputs)
  *   1  brute force with an fp64 chord pre-filter of generous margin, long-double confirm
@@ -130,14 +136,27 @@ typedef struct {
     long double r_l;          /* radius, arcsec, promoted exactly */
     double pre2;              /* pre-filter threshold on chord^2 (generous) */
     int use_pre;
+    const double* errA;       /* per-record error radii in arcsec (both or neither), Eq. (4) */
+    const double* errB;
+    long double k_l;          /* the factor of Eq. (4): 3 in the paper */
+    int self_mode;            /* 0: two catalogues; 1: one catalogue, pairs i < j; 2: pairs i <= j; 3: j != i (nearest) */
 } ctx_t;
 
 /* consider candidate (i, j): confirm in long double; append or update the running best */
 static inline int consider(const ctx_t* c, const double* raA, const double* decA, const int64_t* idA, int64_t i,
                            const double* raB, const double* decB, const int64_t* idB, int64_t j,
                            vec_t* out, pair_t* best, int* have_best) {
+    if (c->self_mode == 1 && !(i < j)) return 0;            /* an unordered pair is reported once, (i, i) never */
+    if (c->self_mode == 2 && !(i <= j)) return 0;
+    if (c->self_mode == 3 && i == j) return 0;
     long double s = sep_arcsec_l(raA[i], decA[i], raB[j], decB[j]);
-    if (!(s <= c->r_l)) return 0;                           /* Eq. (4): inclusive */
+    long double thr = c->r_l;
+    if (c->errA) {                                          /* Eq. (4) per pair: k sqrt(e1^2 + e2^2), capped by the radius */
+        long double e1 = (long double)c->errA[i], e2 = (long double)c->errB[j];
+        long double t = c->k_l * sqrtl(e1 * e1 + e2 * e2);
+        if (t < thr) thr = t;
+    }
+    if (!(s <= thr)) return 0;                              /* Eq. (4): inclusive */
     pair_t p; p.ida = idA ? idA[i] : i; p.idb = idB ? idB[j] : j; p.sep_l = s; p.sep = (double)s;
     if (c->mode == 0) return vec_push(out, p);
     if (!*have_best || s < best->sep_l || (s == best->sep_l && p.idb < best->idb)) { *best = p; *have_best = 1; }
@@ -151,11 +170,36 @@ static inline int consider(const ctx_t* c, const double* raA, const double* decA
  * them with hlc2_oracle_free.  threads <= 0 means "all OpenMP threads"; *threads_used
  * reports what ran.
  */
+int hlc2_oracle_match_ext(const double* raA, const double* decA, const int64_t* idA, int64_t nA,
+                          const double* raB, const double* decB, const int64_t* idB, int64_t nB,
+                          double radius_arcsec, int mode, int engine, int threads,
+                          const double* errA, const double* errB, double k_factor, int self_mode,
+                          int64_t* out_n, int64_t** out_ida, int64_t** out_idb, double** out_sep,
+                          int* threads_used);
+
 int hlc2_oracle_match(const double* raA, const double* decA, const int64_t* idA, int64_t nA,
                       const double* raB, const double* decB, const int64_t* idB, int64_t nB,
                       double radius_arcsec, int mode, int engine, int threads,
                       int64_t* out_n, int64_t** out_ida, int64_t** out_idb, double** out_sep,
                       int* threads_used) {
+    return hlc2_oracle_match_ext(raA, decA, idA, nA, raB, decB, idB, nB, radius_arcsec, mode, engine, threads,
+                                 NULL, NULL, 3.0, 0, out_n, out_ida, out_idb, out_sep, threads_used);
+}
+
+/* The same with per-record error radii (errA, errB: both or neither; arcsec; >= 0) and / or self-match of one catalogue
+ * (self_mode != 0: the caller passes the same arrays as A and B). */
+int hlc2_oracle_match_ext(const double* raA, const double* decA, const int64_t* idA, int64_t nA,
+                          const double* raB, const double* decB, const int64_t* idB, int64_t nB,
+                          double radius_arcsec, int mode, int engine, int threads,
+                          const double* errA, const double* errB, double k_factor, int self_mode,
+                          int64_t* out_n, int64_t** out_ida, int64_t** out_idb, double** out_sep,
+                          int* threads_used) {
+    if ((errA == NULL) != (errB == NULL) || !(k_factor > 0.0) || self_mode < 0 || self_mode > 3 ||
+        (self_mode != 0 && nA != nB)) return ORACLE_BAD_ARG;
+    if (errA) {
+        for (int64_t i = 0; i < nA; ++i) if (!(errA[i] >= 0.0) || !isfinite(errA[i])) return ORACLE_BAD_ARG;
+        for (int64_t j = 0; j < nB; ++j) if (!(errB[j] >= 0.0) || !isfinite(errB[j])) return ORACLE_BAD_ARG;
+    }
     if (nA < 0 || nB < 0 || !(radius_arcsec > 0.0) || !isfinite(radius_arcsec) || radius_arcsec >= 324000.0 ||
         (mode != 0 && mode != 1) || engine < 0 || engine > 2 || !out_n || !out_ida || !out_idb || !out_sep)
         return ORACLE_BAD_ARG;
@@ -163,6 +207,7 @@ int hlc2_oracle_match(const double* raA, const double* decA, const int64_t* idA,
     rc = check_coords(raB, decB, nB); if (rc) return rc;
 
     ctx_t c; c.mode = mode; c.r_l = (long double)radius_arcsec; c.use_pre = engine != 0;
+    c.errA = errA; c.errB = errB; c.k_l = (long double)k_factor; c.self_mode = self_mode;
     {   /* chord of (r + margin): margin = 0.1% of r + 1e-3 arcsec, far above fp64 chord error (~2e-10 arcsec) */
         double r_rad = (radius_arcsec * 1.001 + 1e-3) * (M_PI / 648000.0);
         double ch = 2.0 * sin(0.5 * r_rad);

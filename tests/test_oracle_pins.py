@@ -280,3 +280,96 @@ def test_generators_are_seeded_and_shaped():
     # galactic-plane concentration: fraction of sources within |b| < 10 deg well above the uniform 17.4%
     w = S.config(4, scale=0.002)
     assert (np.abs(w.A.dec) > 89.5).mean() == pytest.approx(0.1, abs=0.01)
+
+
+# ------------------------------------------------------------------------------------------------------
+# extensions: per-record error radii (Eq. (4)) and self-match (L286, L295)
+# ------------------------------------------------------------------------------------------------------
+def _mp_sep_arcsec(ra1, dec1, ra2, dec2):
+    """Eq. (1) itself (law of cosines) in 50-digit arithmetic -- not the oracle's haversine form."""
+    import mpmath as mp
+    mp.mp.dps = 50
+    d2r = mp.pi / 180
+    a1, d1, a2, d2 = (mp.mpf(float(v)) * d2r for v in (ra1, dec1, ra2, dec2))
+    # Vincenty form of the same angle: well conditioned at arcsecond separations
+    num = mp.sqrt((mp.cos(d2) * mp.sin(a2 - a1)) ** 2 + (mp.cos(d1) * mp.sin(d2) - mp.sin(d1) * mp.cos(d2) * mp.cos(a2 - a1)) ** 2)
+    den = mp.sin(d1) * mp.sin(d2) + mp.cos(d1) * mp.cos(d2) * mp.cos(a2 - a1)
+    return mp.atan2(num, den) * 648000 / mp.pi
+
+
+def test_error_radii_hand_cases():
+    """Two equator points 3.6 arcsec apart (theta = dRA exactly).  Eq. (4): 3 sqrt(e1^2 + e2^2)."""
+    ra_a, dec_a = np.array([10.0]), np.array([0.0])
+    ra_b, dec_b = np.array([10.001]), np.array([0.0])                     # 3.6 arcsec
+    for e1, e2, inside in ((1.0, 0.2, False),     # 3 sqrt(1.04) = 3.0594 < 3.6
+                           (1.0, 0.7, True),      # 3 sqrt(1.49) = 3.6620 >= 3.6
+                           (0.0, 1.2, True),      # 3 * 1.2 = 3.6 + 4e-16: the threshold within an ulp of theta -> in or out, so test 1.2000001
+                           (0.0, 1.19, False)):
+        e2 = 1.2000001 if (e1, e2) == (0.0, 1.2) else e2
+        a, b, s, _ = oracle.match(ra_a, dec_a, None, ra_b, dec_b, None, 100.0, 0, oracle.ENGINE_BRUTE_LD,
+                                  err_a=np.array([e1]), err_b=np.array([e2]))
+        assert (len(a) == 1) == inside, (e1, e2, len(a))
+    # a different factor k, and the radius as a cap on the threshold
+    a, *_ = oracle.match(ra_a, dec_a, None, ra_b, dec_b, None, 100.0, 0, 0, err_a=np.array([1.0]), err_b=np.array([0.7]), k_factor=2.0)
+    assert len(a) == 0                                                     # 2 sqrt(1.49) = 2.44
+    a, *_ = oracle.match(ra_a, dec_a, None, ra_b, dec_b, None, 3.5, 0, 0, err_a=np.array([1.0]), err_b=np.array([0.7]))
+    assert len(a) == 0                                                     # threshold 3.66 capped at 3.5 < 3.6
+
+
+def test_error_radii_against_the_written_out_definition():
+    """Random tiny catalogues with random error radii: every pair decided by Eq. (4) with Eq. (1) in 50 digits."""
+    import mpmath as mp
+    rng = np.random.default_rng(77)
+    n = 60
+    ra_a = rng.uniform(30.0, 30.004, n); dec_a = rng.uniform(-60.0, -59.996, n)
+    ra_b = ra_a + rng.normal(0, 2e-4, n); dec_b = dec_a + rng.normal(0, 2e-4, n)
+    ea = rng.uniform(0.05, 0.8, n); eb = rng.uniform(0.05, 0.8, n)
+    want = set()
+    for i in range(n):
+        for j in range(n):
+            th = _mp_sep_arcsec(ra_a[i], dec_a[i], ra_b[j], dec_b[j])
+            thr = 3 * mp.sqrt(mp.mpf(float(ea[i])) ** 2 + mp.mpf(float(eb[j])) ** 2)
+            assert abs(th - thr) > 1e-9                                    # no pair sits on its threshold
+            if th <= thr and th <= 50:
+                want.add((i, j))
+    for eng in (0, 1, 2):
+        a, b, s, _ = oracle.match(ra_a, dec_a, None, ra_b, dec_b, None, 50.0, 0, eng, err_a=ea, err_b=eb)
+        assert set(zip(a.tolist(), b.tolist())) == want and len(want) > 30
+
+
+def test_error_radii_constant_reduces_to_a_single_radius():
+    """e1 = e2 = e for every record: Eq. (4) is the single radius 3 sqrt(2) e (the pinned plain match)."""
+    w = S.config(1, scale=0.05)
+    e = 0.21
+    a0, b0, s0, _ = oracle.match(w.A.ra, w.A.dec, w.A.id, w.B.ra, w.B.dec, w.B.id, 3.0 * np.sqrt(2.0) * e + 1e-12, 0, 2)
+    a1, b1, s1, _ = oracle.match(w.A.ra, w.A.dec, w.A.id, w.B.ra, w.B.dec, w.B.id, 5.0, 0, 2,
+                                 err_a=np.full(len(w.A), e), err_b=np.full(len(w.B), e))
+    assert np.array_equal(a0, a1) and np.array_equal(b0, b1) and np.array_equal(s0, s1) and len(a0) > 1000
+
+
+def test_self_match_is_the_upper_triangle():
+    """One catalogue with exact duplicates: self_mode 1 = the pairs i < j of the full matrix, 2 = those plus the diagonal,
+    3 (nearest) = nearest OTHER source; counts: 2 |upper| + n = |all_pairs(A, A)|."""
+    w = S.config(1, scale=0.05)
+    ra = np.concatenate([w.A.ra, w.A.ra[:40]]); dec = np.concatenate([w.A.dec, w.A.dec[:40]])      # 40 exact duplicates
+    n = len(ra)
+    fa, fb, fs, _ = oracle.match(ra, dec, None, ra, dec, None, 20.0, 0, 2)
+    ua, ub, us, _ = oracle.match(ra, dec, None, ra, dec, None, 20.0, 0, 2, self_mode=oracle.SELF_PAIRS)
+    da, db, ds, _ = oracle.match(ra, dec, None, ra, dec, None, 20.0, 0, 2, self_mode=oracle.SELF_PAIRS_AND_DIAGONAL)
+    up = fa < fb
+    assert np.array_equal(ua, fa[up]) and np.array_equal(ub, fb[up]) and np.array_equal(us, fs[up])
+    assert 2 * len(ua) + n == len(fa) and len(da) == len(ua) + n and (ua < ub).all()
+    dup = set(zip(ua[us == 0.0].tolist(), ub[us == 0.0].tolist()))
+    assert dup == {(i, len(w.A.ra) + i) for i in range(40)}               # each duplicate pair once, no (i, i)
+    # brute force agrees on a slice
+    ba, bb, bs, _ = oracle.match(ra[:400], dec[:400], None, ra[:400], dec[:400], None, 20.0, 0, 0, self_mode=1)
+    va, vb, vs, _ = oracle.match(ra[:400], dec[:400], None, ra[:400], dec[:400], None, 20.0, 0, 2, self_mode=1)
+    assert np.array_equal(ba, va) and np.array_equal(bb, vb)
+    # nearest other source = argmin over the off-diagonal of the full matrix
+    na, nb_, ns, _ = oracle.match(ra, dec, None, ra, dec, None, 20.0, 1, 2, self_mode=oracle.SELF_EXCLUDE_OWN)
+    off = fa != fb
+    best = {}
+    for i, j, s_ in zip(fa[off].tolist(), fb[off].tolist(), fs[off].tolist()):
+        if i not in best or (s_, j) < best[i]:
+            best[i] = (s_, j)
+    assert len(na) == len(best) and all(best[i][1] == j for i, j in zip(na.tolist(), nb_.tolist())) and (na != nb_).all()
