@@ -209,12 +209,15 @@ def run_config5(args, clocks_index=0):
     # band order without the id columns (ids are implicit: the global row numbers of the banded arrays)
     def bands_of(cat):
         k = np.clip(np.searchsorted(edges, cat.dec, side="right") - 1, 0, nb - 1).astype(np.int16)
-        order = np.argsort(k, kind="stable")
         off = np.zeros(nb + 1, np.int64); np.cumsum(np.bincount(k, minlength=nb), out=off[1:])
-        return np.ascontiguousarray(cat.ra[order]), np.ascontiguousarray(cat.dec[order]), off
-    a_ra, a_dec, a_off = bands_of(w.A)
-    b_ra, b_dec, b_off = bands_of(w.B)
+        order = np.argsort(k, kind="stable"); del k
+        ra = cat.ra[order]; dec = cat.dec[order]
+        return ra, dec, off
+    w.planted_a = None; w.planted_b = None               # multi-GB bookkeeping of the generator, not needed here
+    a_ra, a_dec, a_off = bands_of(w.A); w.A = None      # free each original as soon as its banded copy exists
+    b_ra, b_dec, b_off = bands_of(w.B); w.B = None
     del w
+    import gc; gc.collect()
     t_band = time.perf_counter() - t0
     sA = [host_register(a_ra), host_register(a_dec), None]; sB = [host_register(b_ra), host_register(b_dec), None]
     max_a, max_b = int(np.diff(a_off).max()), int(np.diff(b_off).max())

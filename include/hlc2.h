@@ -89,6 +89,8 @@ typedef struct {
     int32_t full_sky;
     int32_t zone_aspect;
     const hlc2_index* grid_like;
+    const double* d_err_arcsec;      /* optional: [n] per-record error radii (device, input order, arcsec, >= 0) for
+                                        hlc2_crossmatch_radii: the r1 / r2 of Eq. (4); NULL = none */
 } hlc2_opts;
 
 /* Description of an index's grid (host data), for tools and for the boundary-stress generator. */
@@ -187,6 +189,32 @@ int hlc2_crossmatch_events(const hlc2_index* A, const hlc2_index* B, double radi
                            int64_t capacity, unsigned long long* d_count,
                            void* d_temp, size_t temp_bytes, void* cuda_stream,
                            void* ev_kernel_start, void* ev_kernel_stop);
+
+/*
+ * Self-match of ONE catalogue (the paper's D4 case: 2MASS against itself, Table 2).
+ *   HLC2_ALL_PAIRS  every unordered pair {i, j}, i != j, within radius_arcsec exactly once (either orientation of
+ *                   (idA, idB); half the tests and half the staging of hlc2_crossmatch(idx, idx)); with
+ *                   include_self != 0 also the n pairs (i, i) at separation 0.
+ *   HLC2_NEAREST    for every source the nearest OTHER source within the radius (a source is not its own neighbour;
+ *                   include_self is ignored).
+ * Other arguments, stream behaviour and scratch size (hlc2_crossmatch_sizes(idx, idx)) as for hlc2_crossmatch.
+ */
+int hlc2_selfmatch(const hlc2_index* idx, double radius_arcsec, int mode, int include_self,
+                   int64_t* d_out_idA, int64_t* d_out_idB, double* d_out_sep_arcsec,
+                   int64_t capacity, unsigned long long* d_count,
+                   void* d_temp, size_t temp_bytes, void* cuda_stream);
+
+/*
+ * Cross-match with the paper's criterion as printed (Eq. (4)): a pair matches when its separation is
+ * <= k_factor * sqrt(r1^2 + r2^2), r1 / r2 the error radii of the two records (both indices must have been built
+ * with opts.d_err_arcsec; k_factor = 3 in the paper), and <= radius_cap_arcsec (the search bound: at most the r_max
+ * of both indices; pass at least k_factor * sqrt(max r1^2 + max r2^2) for the pure Eq. (4)).  Decisions in fp64:
+ * chord^2 <= 4 sin^2(t/2) with t the pair's threshold.  Runs on the general per-lane path.
+ */
+int hlc2_crossmatch_radii(const hlc2_index* A, const hlc2_index* B, double radius_cap_arcsec, double k_factor, int mode,
+                          int64_t* d_out_idA, int64_t* d_out_idB, double* d_out_sep_arcsec,
+                          int64_t capacity, unsigned long long* d_count,
+                          void* d_temp, size_t temp_bytes, void* cuda_stream);
 
 /*
  * Partition streaming from pinned host memory (NS (c); the paper's pinned

@@ -47,7 +47,7 @@ class Hlc2Error(RuntimeError):
 class hlc2_opts(ctypes.Structure):
     _fields_ = [("r_max_arcsec", ctypes.c_double), ("target_occupancy", ctypes.c_double),
                 ("cell_arcsec", ctypes.c_double), ("full_sky", ctypes.c_int32), ("zone_aspect", ctypes.c_int32),
-                ("grid_like", ctypes.c_void_p)]
+                ("grid_like", ctypes.c_void_p), ("d_err_arcsec", ctypes.c_void_p)]
 
 
 class hlc2_grid_info(ctypes.Structure):
@@ -83,6 +83,8 @@ def lib():
         L.hlc2_last_cuda_error.argtypes = [P(ctypes.c_char_p)]
         L.hlc2_kernel_launches.restype = ctypes.c_ulonglong
         L.hlc2_crossmatch_events.argtypes = L.hlc2_crossmatch.argtypes + [vp, vp]
+        L.hlc2_selfmatch.argtypes = [vp, ctypes.c_double, ctypes.c_int, ctypes.c_int, vp, vp, vp, i64, vp, vp, sz, vp]
+        L.hlc2_crossmatch_radii.argtypes = [vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, vp, vp, vp, i64, vp, vp, sz, vp]
         L.hlc2_version.restype = ctypes.c_char_p
         _lib = L
     return _lib
@@ -106,6 +108,7 @@ def make_opts(r_max_arcsec=1.0, target_occupancy=0.0, cell_arcsec=0.0, full_sky=
     o.r_max_arcsec = float(r_max_arcsec); o.target_occupancy = float(target_occupancy)
     o.cell_arcsec = float(cell_arcsec); o.full_sky = int(bool(full_sky)); o.zone_aspect = int(zone_aspect)
     o.grid_like = grid_like.handle if grid_like is not None else None
+    o.d_err_arcsec = None
     return o
 
 
@@ -136,8 +139,9 @@ def hlc2_index_sizes(n: int, opts: hlc2_opts | None = None):
 
 
 def hlc2_build_index(ra_deg, dec_deg, ids=None, opts: hlc2_opts | None = None, stream=None, temp=None,
-                     like: Index | None = None, buf=None) -> Index:
-    """ra_deg, dec_deg: CUDA float64 tensors [n]; ids: CUDA int64 tensor [n] or None (row numbers)."""
+                     like: Index | None = None, buf=None, err_arcsec=None) -> Index:
+    """ra_deg, dec_deg: CUDA float64 tensors [n]; ids: CUDA int64 tensor [n] or None (row numbers);
+    err_arcsec: optional CUDA float64 tensor [n] of per-record error radii (for hlc2_crossmatch_radii)."""
     torch = _torch()
     n = int(ra_deg.shape[0])
     # never write into the caller's options object: it may outlive `like`
@@ -146,6 +150,9 @@ def hlc2_build_index(ra_deg, dec_deg, ids=None, opts: hlc2_opts | None = None, s
     opts = o
     if like is not None:
         opts.grid_like = like.handle
+    if err_arcsec is not None:
+        assert err_arcsec.is_cuda and err_arcsec.dtype == torch.float64 and err_arcsec.is_contiguous() and err_arcsec.shape[0] == n
+        opts.d_err_arcsec = err_arcsec.data_ptr()
     assert ra_deg.is_cuda and dec_deg.is_cuda and ra_deg.dtype == torch.float64 and dec_deg.dtype == torch.float64
     assert ra_deg.is_contiguous() and dec_deg.is_contiguous() and dec_deg.shape[0] == n
     if ids is not None:
@@ -238,6 +245,55 @@ def hlc2_crossmatch(A: Index, B: Index, radius_arcsec: float, mode: int, out_ida
         rc = lib().hlc2_crossmatch_events(*args, e0, e1)
     if rc != HLC2_OK:
         raise Hlc2Error(rc, "hlc2_crossmatch")
+
+
+def _run_sized(call, n_hint: int, dev, capacity):
+    """Allocate outputs, run `call(oa, ob, os, cnt)`, retry once with the exact size if the first buffer was too small."""
+    torch = _torch()
+    cap = int(capacity) if capacity is not None else max(1024, int(n_hint))
+    for _ in range(2):
+        oa = torch.empty(cap, dtype=torch.int64, device=dev); ob = torch.empty(cap, dtype=torch.int64, device=dev)
+        os_ = torch.empty(cap, dtype=torch.float64, device=dev); cnt = torch.zeros(1, dtype=torch.int64, device=dev)
+        call(oa, ob, os_, cnt, cap)
+        found = int(cnt.item())
+        if found <= cap:
+            return oa[:found], ob[:found], os_[:found]
+        cap = found
+    raise RuntimeError("result count changed between runs")
+
+
+def _scratch(A: Index, B: Index):
+    torch = _torch()
+    need = hlc2_crossmatch_sizes(A, B)
+    temp = torch.empty(max(need, 1), dtype=torch.uint8, device=A.buf.device)
+    temp.record_stream(torch.cuda.current_stream())
+    return temp
+
+
+def selfmatch(idx: Index, radius_arcsec: float, mode: int = HLC2_ALL_PAIRS, include_self: bool = False, capacity: int | None = None):
+    """hlc2_selfmatch: every unordered pair of one catalogue once (all_pairs) or the nearest other source (nearest)."""
+    temp = _scratch(idx, idx)
+
+    def call(oa, ob, os_, cnt, cap):
+        rc = lib().hlc2_selfmatch(idx.handle, float(radius_arcsec), int(mode), int(bool(include_self)), oa.data_ptr(), ob.data_ptr(),
+                                  os_.data_ptr(), cap, cnt.data_ptr(), temp.data_ptr(), temp.numel(), _stream_ptr(None))
+        if rc != HLC2_OK:
+            raise Hlc2Error(rc, "hlc2_selfmatch")
+    return _run_sized(call, idx.n, idx.buf.device, capacity)
+
+
+def crossmatch_radii(A: Index, B: Index, radius_cap_arcsec: float, k_factor: float = 3.0, mode: int = HLC2_ALL_PAIRS,
+                     capacity: int | None = None):
+    """hlc2_crossmatch_radii: PAPER.md Eq. (4) per pair, from the error radii the indices were built with."""
+    temp = _scratch(A, B)
+
+    def call(oa, ob, os_, cnt, cap):
+        rc = lib().hlc2_crossmatch_radii(A.handle, B.handle, float(radius_cap_arcsec), float(k_factor), int(mode), oa.data_ptr(),
+                                         ob.data_ptr(), os_.data_ptr(), cap, cnt.data_ptr(), temp.data_ptr(), temp.numel(),
+                                         _stream_ptr(None))
+        if rc != HLC2_OK:
+            raise Hlc2Error(rc, "hlc2_crossmatch_radii")
+    return _run_sized(call, A.n, A.buf.device, capacity)
 
 
 def crossmatch(A: Index, B: Index, radius_arcsec: float, mode: int = HLC2_ALL_PAIRS, capacity: int | None = None):

@@ -38,7 +38,7 @@ struct HostGrid {
 };
 
 struct Layout {           // byte offsets inside the index buffer
-    size_t x, y, z, id, pos, key, cell_start, n_ra, cell_base, tiles, n_tiles, stats, total;
+    size_t x, y, z, id, pos, key, cell_start, n_ra, cell_base, tiles, n_tiles, stats, err2, total;   // err2 = 0: no error radii
     size_t cap_cells, cap_zones, cap_tiles, n_pad;
 };
 struct TempLayout { size_t key_b, perm_a, perm_b, rec, digit_hist, digit_base, ticket, status, big, tile_first, total; };
@@ -124,6 +124,8 @@ static Layout make_layout(int64_t n, const hlc2_opts& o) {
     L.tiles = off; off += align_up(L.cap_tiles * sizeof(TileDesc));
     L.n_tiles = off; off += 256;
     L.stats = off; off += align_up(sizeof(Stats));
+    L.err2 = 0;
+    if (o.d_err_arcsec) { L.err2 = off; off += align_up(L.n_pad * 8); }
     L.total = off;
     return L;
 }
@@ -234,6 +236,7 @@ static IndexView index_view(const hlc2_index* ix) {
     v.x = (const double*)(ix->d_buf + ix->lay.x); v.y = (const double*)(ix->d_buf + ix->lay.y);
     v.z = (const double*)(ix->d_buf + ix->lay.z); v.id = (const int64_t*)(ix->d_buf + ix->lay.id);
     v.pos = (const float2*)(ix->d_buf + ix->lay.pos);
+    v.err2 = ix->lay.err2 ? (const double*)(ix->d_buf + ix->lay.err2) : nullptr;
     v.key = (const uint32_t*)(ix->d_buf + ix->lay.key); v.key_mask = ix->flagged ? kKeyMask : 0xFFFFFFFFu;
     v.cell_start = (const uint32_t*)(ix->d_buf + ix->lay.cell_start);
     v.tiles = (const TileDesc*)(ix->d_buf + ix->lay.tiles); v.n_tiles = (const uint32_t*)(ix->d_buf + ix->lay.n_tiles);
@@ -291,7 +294,7 @@ int hlc2_build_index(const double* d_ra, const double* d_dec, const int64_t* d_i
 
     hlc2_index* ix = new (std::nothrow) hlc2_index();
     if (!ix) return HLC2_ERR_INVALID_ARG;
-    ix->magic = kMagic; ix->n = n; ix->opts = o; ix->opts.grid_like = nullptr; ix->lay = L;
+    ix->magic = kMagic; ix->n = n; ix->opts = o; ix->opts.grid_like = nullptr; ix->opts.d_err_arcsec = nullptr; ix->lay = L;
     ix->d_buf = (char*)d_index_buf; ix->index_bytes = index_bytes; ix->stream = s; ix->stats_valid = false;
     int rc = HLC2_OK;
     auto fail = [&](int code) { delete ix; return code; };
@@ -344,6 +347,7 @@ int hlc2_build_index(const double* d_ra, const double* d_dec, const int64_t* d_i
                                   (uint32_t*)(tmp + T.status), (uint32_t*)(tmp + T.ticket), s);
     const uint32_t* perm = where ? pb : pa;
     launch_gather(rec, perm, nn, (double*)(buf + L.x), (double*)(buf + L.y), (double*)(buf + L.z), (int64_t*)(buf + L.id), (float2*)(buf + L.pos), s);
+    if (L.err2) launch_gather_err2(o.d_err_arcsec, perm, nn, (double*)(buf + L.err2), s);
     launch_cell_table(key_idx, kmask, nn, n_cells, (uint32_t*)(buf + L.cell_start), (uint32_t*)(tmp + T.big), s);
     launch_tiles((const uint32_t*)(buf + L.cell_start), gv.cell_base, gv.n_ra, (uint32_t)g.n_zones, key_idx, kmask,
                  (uint32_t)((size_t)n / kTile + (size_t)g.n_zones + 1), (uint32_t*)(tmp + T.tile_first),
@@ -420,6 +424,42 @@ int hlc2_crossmatch_events(const hlc2_index* A, const hlc2_index* B, double radi
                  (cudaEvent_t)ev_kernel_start, (cudaEvent_t)ev_kernel_stop);
     CU(cudaGetLastError());
     return HLC2_OK;
+}
+
+static int match_extra(const hlc2_index* A, const hlc2_index* B, double radius_arcsec, int mode, const MatchExtra& ex,
+                       int64_t* d_out_idA, int64_t* d_out_idB, double* d_out_sep, int64_t capacity,
+                       unsigned long long* d_count, void* d_temp, size_t temp_bytes, void* cuda_stream) {
+    if (!A || !B || A->magic != kMagic || B->magic != kMagic || !d_count || capacity < 0 ||
+        (capacity > 0 && (!d_out_idA || !d_out_idB || !d_out_sep)) ||
+        (mode != HLC2_ALL_PAIRS && mode != HLC2_NEAREST) ||
+        !(radius_arcsec > 0.0) || !std::isfinite(radius_arcsec)) return HLC2_ERR_INVALID_ARG;
+    if (radius_arcsec > std::min(A->opts.r_max_arcsec, B->opts.r_max_arcsec)) return HLC2_ERR_RADIUS_TOO_LARGE;
+    IndexView va = index_view(A), vb = index_view(B);
+    if (ex.k_factor > 0.0 && (!va.err2 || !vb.err2)) return HLC2_ERR_INVALID_ARG;
+    size_t need = match_temp_bytes(va, vb);
+    if (need > 0 && (!d_temp || temp_bytes < need)) return HLC2_ERR_BUFFER_TOO_SMALL;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    CU(cudaMemsetAsync(d_count, 0, sizeof(unsigned long long), s));
+    launch_match(va, vb, radius_arcsec, mode, d_out_idA, d_out_idB, d_out_sep, (unsigned long long)capacity, d_count,
+                 d_temp, s, same_grid(A, B) ? kMatchSameGrid : 0u, nullptr, nullptr, &ex);
+    CU(cudaGetLastError());
+    return HLC2_OK;
+}
+
+int hlc2_selfmatch(const hlc2_index* idx, double radius_arcsec, int mode, int include_self,
+                   int64_t* d_out_idA, int64_t* d_out_idB, double* d_out_sep, int64_t capacity,
+                   unsigned long long* d_count, void* d_temp, size_t temp_bytes, void* cuda_stream) {
+    MatchExtra ex; ex.k_factor = 0.0;
+    ex.self_mode = mode == HLC2_NEAREST ? 3 : (include_self ? 2 : 1);
+    return match_extra(idx, idx, radius_arcsec, mode, ex, d_out_idA, d_out_idB, d_out_sep, capacity, d_count, d_temp, temp_bytes, cuda_stream);
+}
+
+int hlc2_crossmatch_radii(const hlc2_index* A, const hlc2_index* B, double radius_cap_arcsec, double k_factor, int mode,
+                          int64_t* d_out_idA, int64_t* d_out_idB, double* d_out_sep, int64_t capacity,
+                          unsigned long long* d_count, void* d_temp, size_t temp_bytes, void* cuda_stream) {
+    if (!(k_factor > 0.0) || !std::isfinite(k_factor)) return HLC2_ERR_INVALID_ARG;
+    MatchExtra ex; ex.self_mode = 0; ex.k_factor = k_factor;
+    return match_extra(A, B, radius_cap_arcsec, mode, ex, d_out_idA, d_out_idB, d_out_sep, capacity, d_count, d_temp, temp_bytes, cuda_stream);
 }
 
 int hlc2_crossmatch(const hlc2_index* A, const hlc2_index* B, double radius_arcsec, int mode,

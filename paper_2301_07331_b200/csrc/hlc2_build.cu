@@ -486,6 +486,20 @@ k_cell_fill_big(const uint32_t* __restrict__ big, const uint32_t* __restrict__ b
     }
 }
 
+// per-record error radii (input order, arcsec) -> squares in cell order
+__global__ void __launch_bounds__(256)
+k_gather_err2(const double* __restrict__ err, const uint32_t* __restrict__ perm, uint32_t n, double* __restrict__ err2) {
+    for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (size_t)gridDim.x * 256) {
+        const double e = __ldg(err + __ldg(perm + i));
+        err2[i] = e >= 0.0 ? e * e : __longlong_as_double(0x7ff8000000000000ll);      // a negative or NaN radius matches nothing
+    }
+}
+void launch_gather_err2(const double* err_arcsec, const uint32_t* perm, uint32_t n, double* err2, cudaStream_t s) {
+    if (n == 0) return;
+    int blocks = (int)std::min<size_t>(((size_t)n + 255) / 256, (size_t)sm_count() * 16);
+    k_gather_err2<<<blocks, 256, 0, s>>>(err_arcsec, perm, n, err2); count_launch();
+}
+
 size_t cell_big_cap(size_t n_cells) { return n_cells / kFillWarp + 2; }
 
 void launch_cell_table(const uint32_t* sorted_keys, uint32_t key_mask, uint32_t n, uint32_t n_cells, uint32_t* cell_start,

@@ -63,6 +63,7 @@ struct IndexView {
     const double* x; const double* y; const double* z;   // [n] unit vectors, cell order
     const int64_t* id;                                    // [n]
     const float2* pos;                                    // [n] fp32 (ra, dec) estimate in degrees: locates windows, never decides
+    const double* err2;                                   // [n] squared error radius (arcsec^2) of each sorted row, or null
     const uint32_t* key;                                  // [n] sorted cell keys (& key_mask), window flags in the top bits
     uint32_t key_mask;                                    // kKeyMask when the keys carry flags, else 0xFFFFFFFF
     const uint32_t* cell_start;                           // [n_cells + 1]
@@ -100,12 +101,15 @@ int  launch_radix_sort(uint32_t* keys_a, uint32_t* keys_b, uint32_t* val_a, uint
                        cudaStream_t s);
 void launch_gather(const Rec* rec, const uint32_t* perm, uint32_t n, double* x, double* y, double* z, int64_t* out_id,
                    float2* pos, cudaStream_t s);
+void launch_gather_err2(const double* err_arcsec, const uint32_t* perm, uint32_t n, double* err2, cudaStream_t s);
 size_t cell_big_cap(size_t n_cells);
 void launch_cell_table(const uint32_t* sorted_keys, uint32_t key_mask, uint32_t n, uint32_t n_cells, uint32_t* cell_start,
                        uint32_t* d_big, cudaStream_t s);
 void launch_tiles(const uint32_t* cell_start, const uint32_t* cell_base, const int32_t* n_ra, uint32_t n_zones, const uint32_t* sorted_keys,
                   uint32_t key_mask, uint32_t tile_cap, uint32_t* d_tile_first, TileDesc* tiles, uint32_t* d_n_tiles, cudaStream_t s);
 
+// self-match / per-record radii: self_mode as in MatchArgs; k_factor > 0 switches Eq. (4) per pair on
+struct MatchExtra { int self_mode; double k_factor; };
 size_t match_temp_bytes(const IndexView& A, const IndexView& B);
 constexpr uint32_t kMatchSameGrid = 1u;       // launch_match flag: A and B share one grid and both carry window flags
 size_t match_temp_for_tiles(size_t tile_cap);
@@ -114,7 +118,7 @@ size_t match_temp_bound(int64_t n_a, const hlc2_opts* opts);
 void launch_match(const IndexView& A, const IndexView& B, double radius_arcsec, int mode,
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
                   unsigned long long* d_count, void* d_temp, cudaStream_t s, uint32_t match_flags = 0,
-                  cudaEvent_t ev_start = nullptr, cudaEvent_t ev_stop = nullptr);
+                  cudaEvent_t ev_start = nullptr, cudaEvent_t ev_stop = nullptr, const MatchExtra* ex = nullptr);
 
 void count_launch(int k = 1);
 

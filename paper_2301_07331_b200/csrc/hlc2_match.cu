@@ -473,7 +473,7 @@ size_t match_temp_bytes(const IndexView& A, const IndexView& B) {
 void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_arcsec, int mode,
                   int64_t* out_ida, int64_t* out_idb, double* out_sep, unsigned long long capacity,
                   unsigned long long* d_count, void* d_temp, cudaStream_t s, uint32_t match_flags,
-                  cudaEvent_t ev_start, cudaEvent_t ev_stop) {
+                  cudaEvent_t ev_start, cudaEvent_t ev_stop, const MatchExtra* ex) {
     if (A_in.n == 0 || B_in.n == 0) {
         if (ev_start) cudaEventRecord(ev_start, s);
         if (ev_stop) cudaEventRecord(ev_stop, s);
@@ -484,7 +484,7 @@ void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_ar
     // scanned rows per driving row; measured on config 3 (ratio 2) the two directions tie, so the roles are
     // exchanged only when B is much the smaller catalogue.
     const bool same = (match_flags & kMatchSameGrid) != 0;
-    const bool swap = !same && mode == HLC2_ALL_PAIRS && (size_t)B_in.n * 3 < (size_t)A_in.n;
+    const bool swap = !same && !ex && mode == HLC2_ALL_PAIRS && (size_t)B_in.n * 3 < (size_t)A_in.n;
     const IndexView& A = swap ? B_in : A_in;
     const IndexView& B = swap ? A_in : B_in;
     if (swap) std::swap(out_ida, out_idb);
@@ -497,6 +497,17 @@ void launch_match(const IndexView& A_in, const IndexView& B_in, double radius_ar
     p.sin_r_up = (float)((double)sinl(r_rad) * (1.0 + 1e-5));
     p.out_ida = out_ida; p.out_idb = out_idb; p.out_sep = out_sep; p.capacity = capacity; p.count = d_count;
     p.jobs = nullptr; p.pool_count = nullptr; p.tile_cap = 0; p.pool_cap = 0;
+    p.self_mode = ex ? ex->self_mode : 0;
+    p.ea2 = nullptr; p.eb2 = nullptr; p.kfac2rad = 0.0;
+    if (ex && ex->k_factor > 0.0) {
+        p.ea2 = A.err2; p.eb2 = B.err2;
+        const long double f = (long double)ex->k_factor * (3.141592653589793238462643383279502884L / 648000.0L);
+        p.kfac2rad = (double)(f * f);
+    }
+    if (p.eb2 || (p.self_mode && !same)) {     // per-record radii, or a self-match off the same-grid kernel: the general per-lane path
+        launch_match_all_general(A, B, p, mode, s, ev_start, ev_stop);
+        return;
+    }
     if (same) {         // both indices on one grid: no planner, no job records (hlc2_match_same.cu)
         launch_match_same(A, B, p, mode, d_temp, s, ev_start, ev_stop);
         return;

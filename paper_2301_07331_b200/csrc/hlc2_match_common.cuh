@@ -33,7 +33,19 @@ struct MatchArgs {
     Job* jobs;            // [tile_cap] first jobs, then [pool_cap] chained jobs
     uint32_t* pool_count;
     uint32_t tile_cap, pool_cap;
+    // one catalogue matched with itself (PAPER.md D4, L286, L295): 0 no; 1 every unordered pair once (B row > A row);
+    // 2 those and the diagonal (B row >= A row); 3 every B row but the A row itself (nearest: not its own neighbour)
+    int self_mode;
+    // per-record error radii (Eq. (4)): squares in arcsec^2 in cell order, or null; threshold of a pair =
+    // min(radius, k sqrt(e1^2 + e2^2)), k^2 (pi / 648000)^2 folded into kfac2rad
+    const double* ea2; const double* eb2; double kfac2rad;
 };
+
+// 4 sin^2(t / 2) from t^2 (radians^2): t^2 - t^4/12 + t^6/360 - t^8/20160; the next term is below 1e-14 relative up to
+// t = 10 degrees (the largest radius an index accepts)
+__device__ __forceinline__ double chord2_of_angle2(double t2) {
+    return t2 * fma(t2, fma(t2, fma(t2, -1.0 / 20160.0, 1.0 / 360.0), -1.0 / 12.0), 1.0);
+}
 
 // ---- mbarrier / bulk-copy primitives (sm_90+ PTX) ----------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -104,10 +116,14 @@ __device__ __forceinline__ void emit_direct(const IndexView& A, const IndexView&
 template <int MODE>
 __device__ __forceinline__ void scan_global(const IndexView& A, const IndexView& B, const MatchArgs& p, uint32_t a_row,
                                             double ax, double ay, double az, uint32_t j0, uint32_t j1, Best& h) {
+    if (p.self_mode == 1) j0 = max(j0, a_row + 1u); else if (p.self_mode == 2) j0 = max(j0, a_row);
+    const double ea2 = p.eb2 ? __ldg(p.ea2 + a_row) : 0.0;
     for (uint32_t j = j0; j < j1; ++j) {
+        if (p.self_mode == 3 && j == a_row) continue;
         const double dx = ax - __ldg(B.x + j), dy = ay - __ldg(B.y + j), dz = az - __ldg(B.z + j);
         const double c2 = fma(dx, dx, fma(dy, dy, dz * dz));
-        if (c2 <= p.thr2) {
+        const double thr2 = p.eb2 ? fmin(p.thr2, chord2_of_angle2((ea2 + __ldg(p.eb2 + j)) * p.kfac2rad)) : p.thr2;
+        if (c2 <= thr2) {
             if (MODE == HLC2_ALL_PAIRS) emit_direct(A, B, p, a_row, j, c2);
             else if (!h.has || c2 < h.c2 || (c2 == h.c2 && __ldg(B.id + j) < __ldg(B.id + h.row))) { h.has = true; h.row = j; h.c2 = c2; }
         }
@@ -188,6 +204,8 @@ __device__ __forceinline__ void push_hits(const IndexView& A, const IndexView& B
 
 // launchers of the same-grid path (hlc2_match_same.cu)
 size_t match_same_temp_bytes(const IndexView& A);
+void launch_match_all_general(const IndexView& A, const IndexView& B, const MatchArgs& p, int mode, cudaStream_t s,
+                              cudaEvent_t ev_start, cudaEvent_t ev_stop);
 void launch_match_same(const IndexView& A, const IndexView& B, const MatchArgs& p, int mode, void* d_temp, cudaStream_t s,
                        cudaEvent_t ev_start, cudaEvent_t ev_stop);
 

@@ -362,9 +362,13 @@ k_match_same(const __grid_constant__ IndexView A, const __grid_constant__ IndexV
         const int elo = (int)((kf >> 28) & 1u), ehi = (int)((kf >> 29) & 1u);
         bool act = mine && !general;
         uint32_t c0, c1;                   // the lane's cells as global cell numbers [c0, c1]
-        if ((flags & (kSLo | kSHi)) == 0u) { c0 = key - (uint32_t)elo; c1 = key + (uint32_t)ehi; }
-        else {
+        uint32_t self_lo = 0;              // self-match, every unordered pair once: only B rows behind the A row count
+        if ((flags & (kSLo | kSHi)) == 0u) {
+            c0 = key - (uint32_t)elo; c1 = key + (uint32_t)ehi;
+            if (p.self_mode == 1) self_lo = a_row + 1u; else if (p.self_mode == 2) self_lo = a_row;
+        } else {
             act = act && (kf & ((flags & kSLo) ? kKeyDecLo : kKeyDecHi)) != 0u;
+            if ((flags & kSLo) && (p.self_mode == 1 || p.self_mode == 2)) act = false;      // the zone below holds earlier rows only
             const int k = (int)(key - st.d.cb_own);
             c0 = st.d.cb_nb + (uint32_t)nb_first(k - elo, st.d.c_lo); c1 = st.d.cb_nb + (uint32_t)nb_last(k + ehi, (int)dw.y, st.d.c_hi);
         }
@@ -374,8 +378,8 @@ k_match_same(const __grid_constant__ IndexView A, const __grid_constant__ IndexV
         } else {
             unsigned p0 = 0, len = 0;
             if (act) {
-                const uint32_t q0 = min(max(st.cs[c0 - dv.y], dv.w), dw.x);
                 const uint32_t q1 = min(max(st.cs[c1 + 1u - dv.y], dv.w), dw.x);
+                const uint32_t q0 = min(max(max(st.cs[c0 - dv.y], dv.w), self_lo), q1);
                 p0 = q0 - dv.z; len = q1 - q0;
             }
             const unsigned mx = __reduce_max_sync(kFull, len);
@@ -386,9 +390,9 @@ k_match_same(const __grid_constant__ IndexView A, const __grid_constant__ IndexV
                 const unsigned j = p0 + i;
                 const double dx = ax - st.bx[j], dy = ay - st.by[j], dz = az - st.bz[j];
                 const double c2v = fma(dx, dx, fma(dy, dy, dz * dz));
-                const bool hit = in && c2v <= p.thr2;
+                const uint32_t r = j + dv.z;
+                const bool hit = in && c2v <= p.thr2 && (p.self_mode != 3 || r != a_row);
                 if (hit) {
-                    const uint32_t r = j + dv.z;
                     if (MODE == HLC2_ALL_PAIRS) {
                         // a lane holds its first pair of the tile (queued with everybody's at the tile's end: one ballot per
                         // tile instead of one per step); a second pair for the same A row is rare and goes straight out
@@ -408,6 +412,28 @@ k_match_same(const __grid_constant__ IndexView A, const __grid_constant__ IndexV
     }
     __syncwarp();
     ring_drain_rows(A, B, p, w, os.head, os.tail, os.pend, os.base0, os.base1, lane);
+}
+
+// every A row through the general per-lane path (per-record radii; a self-match whose grid does not qualify for the
+// same-grid kernel): one lane per row, windows from the fp32 estimate, B through L2
+template <int MODE>
+__global__ void __launch_bounds__(256)
+k_match_all_general(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B, const __grid_constant__ MatchArgs p) {
+    for (uint32_t row = blockIdx.x * 256 + threadIdx.x; row < A.n; row += gridDim.x * 256) {
+        Best h; h.has = false; h.c2 = 0.0; h.row = 0;
+        scan_general<MODE>(A, B, p, row, __ldg(A.x + row), __ldg(A.y + row), __ldg(A.z + row), __ldg(A.pos + row), h);
+        if (MODE == HLC2_NEAREST && h.has) emit_direct(A, B, p, row, h.row, h.c2);
+    }
+}
+
+void launch_match_all_general(const IndexView& A, const IndexView& B, const MatchArgs& p, int mode, cudaStream_t s,
+                              cudaEvent_t ev_start, cudaEvent_t ev_stop) {
+    const unsigned blocks = (unsigned)std::max<size_t>(1, std::min<size_t>(((size_t)A.n + 255) / 256, (size_t)sm_count() * 8));
+    if (ev_start) cudaEventRecord(ev_start, s);
+    if (mode == HLC2_NEAREST) k_match_all_general<HLC2_NEAREST><<<blocks, 256, 0, s>>>(A, B, p);
+    else                      k_match_all_general<HLC2_ALL_PAIRS><<<blocks, 256, 0, s>>>(A, B, p);
+    count_launch();
+    if (ev_stop) cudaEventRecord(ev_stop, s);
 }
 
 size_t match_same_temp_bytes(const IndexView& A) { return 256 + (size_t)A.n * sizeof(uint32_t); }
