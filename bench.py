@@ -186,43 +186,65 @@ def host_register(arr):
     return torch.from_numpy(arr)
 
 
-def run_config5(args, clocks_index=0):
-    """Configuration 5 ("Streamed large", nearest): the catalogues never sit in HBM as a whole; one step = one call of
-    hlc2_stream_crossmatch over all declination bands from pinned host memory (H2D of the next bands, index build + match
-    of the current one and D2H of the previous one's rows overlap on three streams).  Bound by the PCIe link, so the
-    roofline is the measured pinned copy rate.  At scale 1 the pinned inputs are 48 GB (ids implicit) and generation
-    takes a quarter of an hour on the box's 16 cores; --scale states the fraction actually run."""
+def transfer_model(gib=1):
+    """alpha and beta of PAPER.md Eq. (5), T(d) = alpha + beta d, measured as the paper prescribes (L204-208): alpha = the
+    time of a one-byte transfer, beta = (t_s - alpha) / s for one large transfer (here 1 GiB), pinned memory, per direction."""
+    import torch
+    big = gib << 30
+    h1 = torch.empty(1, dtype=torch.uint8).pin_memory(); d1 = torch.empty(1, dtype=torch.uint8, device="cuda")
+    hb = torch.empty(big, dtype=torch.uint8).pin_memory(); db = torch.empty(big, dtype=torch.uint8, device="cuda")
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    out = {}
+    for name, (s1, t1, sb, tb) in {"h2d": (h1, d1, hb, db), "d2h": (d1, h1, db, hb)}.items():
+        for _ in range(20): t1.copy_(s1, non_blocking=True)
+        torch.cuda.synchronize()
+        e0, e1 = ev(), ev(); e0.record()
+        for _ in range(200): t1.copy_(s1, non_blocking=True)
+        e1.record(); e1.synchronize()
+        alpha = e0.elapsed_time(e1) * 1e-3 / 200
+        best = 1e9
+        for _ in range(3):
+            e0, e1 = ev(), ev(); e0.record(); tb.copy_(sb, non_blocking=True); e1.record(); e1.synchronize()
+            best = min(best, e0.elapsed_time(e1) * 1e-3)
+        out[name] = {"alpha_s": alpha, "beta_s_per_byte": (best - alpha) / big, "gbs": big / best / 1e9}
+    return out
+
+
+def run_streamed(args, w, label, mode, nb, clocks_index=0, extra=None, paper=None):
+    """One step = one call of hlc2_stream_crossmatch over all declination bands from pinned host memory (H2D of the next
+    bands, index build + match of the current one and D2H of the previous one's rows overlap on three streams): the
+    catalogues never sit in HBM as a whole.  Bound by the PCIe link, so the roofline is the measured pinned copy rate.
+    Also fits the paper's cost model (Eq. (5)-(6), L204-214) on this machine and compares its prediction."""
+    import gc
     import torch
     import hlc2_synth as S
     import paper_2301_07331_b200 as P
     import oracle
     from tests import parity
-    scale = args.scale
-    t0 = time.perf_counter()
-    w = S.config(5, scale=scale)
-    t_gen = time.perf_counter() - t0
-    n_a, n_b, r, mode = len(w.A), len(w.B), w.radius_arcsec, 1
-    nb = args.bands
+    n_a, n_b, r = len(w.A), len(w.B), w.radius_arcsec
+    lo_d, hi_d = float(w.A.dec.min()), float(w.A.dec.max())
     edges = np.quantile(w.A.dec[:: max(1, n_a // 2_000_000)], np.linspace(0.0, 1.0, nb + 1))
     edges[0], edges[-1] = -90.0, 90.0
+    edges = np.maximum.accumulate(edges)
+    for k in range(1, nb + 1):                              # bands at least 2 r high (a narrow strip: fewer, equal bands)
+        if edges[k] - edges[k - 1] < 2.0 * r / 3600.0:
+            edges = np.concatenate([[-90.0], np.linspace(lo_d, hi_d, nb + 1)[1:-1], [90.0]]); break
     t0 = time.perf_counter()
-    # band order without the id columns (ids are implicit: the global row numbers of the banded arrays)
-    def bands_of(cat):
+    def bands_of(cat):         # band order without the id columns (ids are implicit: the global row numbers of the banded arrays)
         k = np.clip(np.searchsorted(edges, cat.dec, side="right") - 1, 0, nb - 1).astype(np.int16)
         off = np.zeros(nb + 1, np.int64); np.cumsum(np.bincount(k, minlength=nb), out=off[1:])
         order = np.argsort(k, kind="stable"); del k
         ra = cat.ra[order]; dec = cat.dec[order]
         return ra, dec, off
-    w.planted_a = None; w.planted_b = None               # multi-GB bookkeeping of the generator, not needed here
-    a_ra, a_dec, a_off = bands_of(w.A); w.A = None      # free each original as soon as its banded copy exists
+    w.planted_a = None; w.planted_b = None                 # multi-GB bookkeeping of the generator, not needed here
+    a_ra, a_dec, a_off = bands_of(w.A); w.A = None          # free each original as soon as its banded copy exists
     b_ra, b_dec, b_off = bands_of(w.B); w.B = None
-    del w
-    import gc; gc.collect()
+    del w; gc.collect()
     t_band = time.perf_counter() - t0
     sA = [host_register(a_ra), host_register(a_dec), None]; sB = [host_register(b_ra), host_register(b_dec), None]
     max_a, max_b = int(np.diff(a_off).max()), int(np.diff(b_off).max())
-    cap = int(0.45 * n_a) + 1024
-    mbo = max_a
+    cap = int(0.45 * n_a) + 1024 if mode == 1 else int(1.1 * min(n_a, n_b)) + 1_000_000
+    mbo = max(max_a, max_b)
     opts = P.make_opts(r, target_occupancy=args.occupancy)
     arena = torch.empty(P.hlc2_stream_sizes(max_a, max_b, opts, mbo), dtype=torch.uint8, device="cuda")
     h_out = [torch.empty(cap, dtype=torch.int64).pin_memory(), torch.empty(cap, dtype=torch.int64).pin_memory(),
@@ -236,47 +258,176 @@ def run_config5(args, clocks_index=0):
     clocks = ClockSampler(clocks_index); clocks.start()
     n0 = P.kernel_launches()
     torch.cuda.synchronize()
+    t_wall = time.perf_counter()
     e0, e1 = ev(), ev(); e0.record()
     for _ in range(args.steps):
         found = step()
     e1.record(); torch.cuda.synchronize()
+    t_wall = (time.perf_counter() - t_wall) / args.steps
     launches = P.kernel_launches() - n0
     clk = clocks.stop()
     t_ms = e0.elapsed_time(e1) / args.steps
-    pcie = pcie_rates()
     h2d, d2h = 16 * (n_a + n_b), 24 * found
-    t_pcie = max(h2d / (pcie["h2d_gbs"] * 1e9), d2h / (pcie["d2h_gbs"] * 1e9))
-    # ---- parity on a stated sample of bands: every 16th, both polar bands, and the bands next to them
+    # ---- parity on a stated sample of bands: every 16th, both end bands, and the bands next to them
     ga = h_out[0][:found].numpy(); gb_ = h_out[1][:found].numpy(); gs = h_out[2][:found].numpy()
     sample = sorted(set(list(range(0, nb, 16)) + [0, 1, nb - 2, nb - 1]) & set(range(nb)))
-    ver = {"bands_checked": sample, "rows_gpu": 0, "rows_oracle": 0, "only_gpu": 0, "only_oracle": 0, "borderline": 0, "swaps": 0, "max_sep_err": 0.0}
+    ver = {"bands_checked": sample, "rows_gpu": 0, "rows_oracle": 0, "borderline": 0, "swaps": 0, "max_sep_err": 0.0}
     t_or = 0.0; used = 0
+    cmp = parity.compare_nearest if mode == 1 else parity.compare_all_pairs
     for k in sample:
         a0, a1 = int(a_off[k]), int(a_off[k + 1]); lo, hi = max(k - 1, 0), min(k + 1, nb - 1)
         b0, b1 = int(b_off[lo]), int(b_off[hi + 1])
+        if a1 == a0: continue
         A = S.Catalogue(a_ra[a0:a1], a_dec[a0:a1], np.arange(a0, a1, dtype=np.int64)); B = S.Catalogue(b_ra[b0:b1], b_dec[b0:b1], np.arange(b0, b1, dtype=np.int64))
         t1 = time.perf_counter()
         oa, ob, os_, used = oracle.match(A.ra, A.dec, A.id, B.ra, B.dec, B.id, r, mode)
         t_or += time.perf_counter() - t1
         m = (ga >= a0) & (ga < a1)
-        rep = parity.compare_nearest((ga[m], gb_[m], gs[m]), (oa, ob, os_), r, parity.make_sep_of(A, B))
+        rep = cmp((ga[m], gb_[m], gs[m]), (oa, ob, os_), r, parity.make_sep_of(A, B))     # raises on any lost / invented pair
         ver["rows_gpu"] += int(m.sum()); ver["rows_oracle"] += len(oa)
         ver["borderline"] += len(rep["borderline"]); ver["swaps"] += len(rep.get("swaps", []))
         ver["max_sep_err"] = max(ver["max_sep_err"], float(rep["max_sep_err"]))
     a_checked = int(sum(a_off[k + 1] - a_off[k] for k in sample))
+    # ---- the paper's cost model on this machine (Eq. (5)-(6)): transfer alpha / beta, device term sigma + c n fitted on
+    # resident runs of 1, 2 and 4 merged bands from the middle of the sky
+    tm = transfer_model()
+    pts = []
+    mid = nb // 2
+    for g in (1, 2, 4):
+        k0, k1 = max(0, mid - g // 2), min(nb, max(0, mid - g // 2) + g)
+        a0, a1, b0, b1 = int(a_off[k0]), int(a_off[k1]), int(b_off[k0]), int(b_off[k1])
+        if a1 - a0 < 1000 or b1 - b0 < 1000: continue
+        da = [torch.from_numpy(a_ra[a0:a1]).cuda(), torch.from_numpy(a_dec[a0:a1]).cuda()]
+        db = [torch.from_numpy(b_ra[b0:b1]).cuda(), torch.from_numpy(b_dec[b0:b1]).cuda()]
+        oc = torch.empty(a1 - a0 + b1 - b0, dtype=torch.int64, device="cuda"); od = torch.empty_like(oc); os2 = torch.empty(oc.shape[0], dtype=torch.float64, device="cuda")
+        cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+        ts = []
+        for rep_ in range(4):
+            f0, f1 = ev(), ev(); f0.record()
+            ib = P.hlc2_build_index(db[0], db[1], None, opts=opts); ia = P.hlc2_build_index(da[0], da[1], None, opts=opts, like=ib)
+            P.hlc2_crossmatch(ia, ib, r, mode, oc, od, os2, cnt)
+            f1.record(); f1.synchronize()
+            if rep_: ts.append(f0.elapsed_time(f1) * 1e-3)
+        pts.append((a1 - a0 + b1 - b0, float(np.median(ts))))
+        del da, db, oc, od, os2
+    model = {"transfer": tm}
+    if len(pts) >= 2:
+        xs, ys = np.array([p_[0] for p_ in pts], float), np.array([p_[1] for p_ in pts], float)
+        c_dev, sigma = np.polyfit(xs, ys, 1)
+        na_k, nb_k = np.diff(a_off).astype(float), np.diff(b_off).astype(float)
+        win_k = nb_k.copy()          # (the window also holds a thin halo of its neighbours: negligible for the model)
+        t_in = tm["h2d"]["alpha_s"] * 2 * nb + tm["h2d"]["beta_s_per_byte"] * 16.0 * (na_k + nb_k).sum()
+        t_dev = float((sigma + c_dev * (na_k + win_k)).sum())
+        t_out = tm["d2h"]["alpha_s"] * 3 * nb + tm["d2h"]["beta_s_per_byte"] * 24.0 * found
+        model.update({"device_fit": {"points_n_seconds": pts, "sigma_s": float(sigma), "seconds_per_source": float(c_dev)},
+                      "eq6_sum_ms": 1e3 * (t_in + t_dev + t_out), "overlapped_max_ms": 1e3 * max(t_in, t_dev, t_out),
+                      "terms_ms": {"transfer_in": 1e3 * t_in, "device": 1e3 * t_dev, "transfer_out": 1e3 * t_out},
+                      "measured_ms": t_ms,
+                      "note": "Eq. (6) adds the terms of every round (the paper's upper limit, no overlap); with the three streams overlapped the step should take about the largest term"})
+    t_pcie = max(tm["h2d"]["beta_s_per_byte"] * h2d, tm["d2h"]["beta_s_per_byte"] * d2h)
+    cfg = {"workload": label, "n_a": n_a, "n_b": n_b, "radius_arcsec": r, "mode": "nearest" if mode else "all_pairs",
+           "rows_found": int(found), "bands": nb, "max_band_a": max_a, "max_band_b": max_b, "arena_bytes": int(arena.numel()),
+           "ids": "implicit (global row numbers of the banded arrays)", "band_seconds": t_band}
+    cfg.update(extra or {})
     line = {"metric": METRIC, "value": n_a / (t_ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": t_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "cfg5_streamed_large", "scale": scale, "n_a": n_a, "n_b": n_b, "radius_arcsec": r, "mode": "nearest",
-                       "rows_found": int(found), "bands": nb, "max_band_a": max_a, "max_band_b": max_b, "arena_bytes": int(arena.numel()),
-                       "ids": "implicit (global row numbers of the banded arrays)", "gen_seconds": t_gen, "band_seconds": t_band,
-                       "note": "scale 1 = 2e9 x 1e9; the fraction run is stated here"},
+            "ms_per_step": t_ms, "wall_s_per_step": t_wall, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": cfg,
             "e2e": {"value": n_a / (t_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "path": "pinned host bands -> hlc2_stream_crossmatch (H2D, build, match, D2H overlapped on 3 streams)"},
-            "roofline": {"bound": "pcie", "achieved": h2d / (t_ms * 1e-3) / 1e9, "peak": pcie["h2d_gbs"], "unit": "GB/s",
-                         "frac": (h2d / (t_ms * 1e-3) / 1e9) / pcie["h2d_gbs"], "traffic": None, "pcie": pcie, "ms_at_peak": 1e3 * t_pcie},
+            "roofline": {"bound": "pcie", "achieved": h2d / (t_ms * 1e-3) / 1e9, "peak": tm["h2d"]["gbs"], "unit": "GB/s",
+                         "frac": (h2d / (t_ms * 1e-3) / 1e9) / tm["h2d"]["gbs"], "traffic": None, "ms_at_peak": 1e3 * t_pcie},
             "cpu_baseline": {"value": a_checked / t_or if t_or else None, "unit": UNIT, "cores": used, "kind": "oracle",
                              "sample": f"the {len(sample)} checked bands: {a_checked} A sources against their three-band B windows"},
-            "verify": ver, "gpu_launches": int(launches), "clocks": clk}
+            "verify": ver, "model": model, "paper_context": paper, "gpu_launches": int(launches), "clocks": clk}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+def run_config5(args, clocks_index=0):
+    """Configuration 5 ("Streamed large", nearest).  At scale 1 the pinned inputs are 48 GB (ids implicit) and generation
+    takes minutes on the box's 16 cores; --scale states the fraction actually run."""
+    import hlc2_synth as S
+    t0 = time.perf_counter()
+    w = S.config(5, scale=args.scale)
+    t_gen = time.perf_counter() - t0
+    return run_streamed(args, w, "cfg5_streamed_large", 1, args.bands, clocks_index,
+                        extra={"scale": args.scale, "gen_seconds": t_gen, "note": "scale 1 = 2e9 x 1e9; the fraction run is stated here"})
+
+
+def run_shape(args, clocks_index=0):
+    """End to end from host arrays at the shapes of the paper's data sets (Table 2), beside its own times
+    (Table 5: P100 / V100, file I/O included, radius not stated) -- context, not a target.  Synthetic stand-ins:
+    D2 = two 1 105 627-source catalogues in the strip RA [340, 360], Dec [1, 1.2]; D4 = 61 734 000 sources of a
+    galactic-plane-concentrated full sky matched with themselves; D6 = 467 555 800 x 102 890 000 sources of the same sky."""
+    import torch
+    import hlc2_synth as S
+    import paper_2301_07331_b200 as P
+    import oracle
+    from tests import parity
+    shape = args.shape
+    t0 = time.perf_counter()
+    if shape == "D2":
+        n = 1_105_627
+        samp = lambda rng, m: S.uniform_patch(rng, m, 340.0, 360.0, 1.0, 1.2)
+        w = S.custom("shape_D2_1105627x1105627_strip", S.BASE_SEED + 12, n, int(0.7 * n), n - int(0.7 * n), samp, 0.3, 1.0, ("all_pairs",))
+        return run_streamed(args, w, w.name, 0, 4, clocks_index, extra={"gen_seconds": time.perf_counter() - t0},
+                            paper={"table5": "HLC2 5 s (1105627 x 1105627), P100 / V100, files included", "line": "P:L368"})
+    if shape == "D6":
+        na, nb_ = 467_555_800, 102_890_000
+        w = S.custom("shape_D6_467555800x102890000_fullsky", S.BASE_SEED + 16, na, int(0.6 * nb_), nb_ - int(0.6 * nb_), S.galactic_density, 0.2, 1.0, ("all_pairs",))
+        return run_streamed(args, w, w.name, 0, 128, clocks_index, extra={"gen_seconds": time.perf_counter() - t0},
+                            paper={"table5": "HLC2 260 s (467555800 x 102890000), P100 / V100, files included", "line": "P:L368"})
+    assert shape == "D4"
+    n, r = 61_734_000, 1.0
+    w = S.custom("shape_D4_61734000_self", S.BASE_SEED + 14, n, 0, 1, S.galactic_density, 0.2, r, ("all_pairs",))
+    t_gen = time.perf_counter() - t0
+    h = [torch.from_numpy(w.A.ra).pin_memory(), torch.from_numpy(w.A.dec).pin_memory()]
+    opts = P.make_opts(r)
+    ib, tb = P.hlc2_index_sizes(n, opts)
+    buf = torch.empty(ib, dtype=torch.uint8, device="cuda"); temp = torch.empty(tb, dtype=torch.uint8, device="cuda")
+    cap = n // 8 + 1024
+    oa = torch.empty(cap, dtype=torch.int64, device="cuda"); ob = torch.empty_like(oa); os_ = torch.empty(cap, dtype=torch.float64, device="cuda")
+    cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ho = [torch.empty(cap, dtype=torch.int64).pin_memory(), torch.empty(cap, dtype=torch.int64).pin_memory(), torch.empty(cap, dtype=torch.float64).pin_memory()]
+    idx = P.hlc2_build_index(h[0].cuda(), h[1].cuda(), None, opts=opts, temp=temp, buf=buf)
+    mtemp = torch.empty(max(1, P.hlc2_crossmatch_sizes(idx, idx)), dtype=torch.uint8, device="cuda")
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    def step(marks=None):
+        d = [t.cuda(non_blocking=True) for t in h]
+        if marks: marks[0].record()
+        ix = P.hlc2_build_index(d[0], d[1], None, opts=opts, temp=temp, buf=buf)
+        if marks: marks[1].record()
+        rc = P.lib().hlc2_selfmatch(ix.handle, r, 0, 0, oa.data_ptr(), ob.data_ptr(), os_.data_ptr(), cap, cnt.data_ptr(), mtemp.data_ptr(), mtemp.numel(), None)
+        assert rc == 0
+        if marks: marks[2].record()
+        nf = int(cnt.item())
+        for src, dst in zip((oa, ob, os_), ho): dst[:nf].copy_(src[:nf], non_blocking=True)
+        return nf
+    for _ in range(3): nf = step()
+    torch.cuda.synchronize()
+    marks = [ev(), ev(), ev()]
+    e0, e1 = ev(), ev(); e0.record()
+    for k in range(args.steps): nf = step(marks if k == args.steps - 1 else None)
+    e1.record(); torch.cuda.synchronize()
+    t_ms = e0.elapsed_time(e1) / args.steps
+    # parity on a 6-degree RA slice: the slice's pairs from the oracle's self-match against the GPU rows of those sources
+    m = (w.A.ra >= 100.0) & (w.A.ra < 106.0); rows = np.flatnonzero(m)
+    A = S.Catalogue(w.A.ra[rows], w.A.dec[rows], rows.astype(np.int64))
+    o_a, o_b, o_s, used = oracle.match(A.ra, A.dec, A.id, A.ra, A.dec, A.id, r, 0, self_mode=oracle.SELF_PAIRS)
+    ga, gb_, gs = ho[0][:nf].numpy(), ho[1][:nf].numpy(), ho[2][:nf].numpy()
+    inside = m[ga] & m[gb_]
+    lo = lambda x, y: (np.minimum(x, y), np.maximum(x, y))
+    g = lo(ga[inside], gb_[inside]); o = lo(o_a, o_b)
+    rep = parity.compare_all_pairs((g[0], g[1], gs[inside]), (o[0], o[1], o_s), r, parity.make_sep_of(A, A))
+    line = {"metric": METRIC, "value": n / (t_ms * 1e-3), "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": 3, "ms_per_step": t_ms,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "n_a": n, "n_b": n, "radius_arcsec": r, "mode": "self-match, every unordered pair once", "rows_found": int(nf),
+                       "gen_seconds": t_gen, "path": "pinned host -> H2D -> hlc2_build_index -> hlc2_selfmatch -> D2H of count and rows"},
+            "phases_ms": {"build_index": marks[0].elapsed_time(marks[1]), "selfmatch": marks[1].elapsed_time(marks[2])},
+            "e2e": {"value": n / (t_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 16 * n, "d2h_bytes_per_step": 24 * nf + 8},
+            "verify": {"against": "oracle self-match on the RA slice [100, 106) deg", "n_gpu": rep["n_gpu"], "n_oracle": rep["n_oracle"],
+                       "borderline": len(rep["borderline"]), "max_sep_err": float(rep["max_sep_err"])},
+            "paper_context": {"table5": "HLC2 150 s (61734000 x 61734000), P100 / V100, files included", "line": "P:L368"}}
     print(json.dumps(line), flush=True)
     return 0
 
@@ -297,6 +448,7 @@ def main():
     ap.add_argument("--occupancy-b", type=float, default=None, help="target occupancy of B's index (default: same as --occupancy)")
     ap.add_argument("--bands", type=int, default=16, help="declination bands of the streamed e2e leg")
     ap.add_argument("--no-stream", action="store_true", help="skip the streamed e2e leg")
+    ap.add_argument("--shape", default=None, choices=["D2", "D4", "D6"], help="end to end at the shape of one of the paper's data sets (Table 2) instead of a configuration")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank, local_rank, world = dist_env()
@@ -304,11 +456,13 @@ def main():
     import hlc2_synth as S
     if args.impl == "reference" and rank != 0:
         return 0
-    if args.config == 5 and args.impl == "ours":
+    if (args.config == 5 or args.shape) and args.impl == "ours":
         import torch
         from paper_2301_07331_b200 import build as hb
         hb.build()
         torch.cuda.set_device(local_rank)
+        if args.shape:
+            return run_shape(args, local_rank)
         if args.bands == 16: args.bands = 64
         return run_config5(args, local_rank)
     t0 = time.perf_counter()

@@ -321,6 +321,12 @@ def config(k: int, scale: float = 1.0, grid: dict | None = None, seed: int | Non
     raise ValueError(f"unknown config {k}")
 
 
+def custom(name, seed, n_a, n_copy, n_extra, sampler, sigma_arcsec, radius_arcsec, modes=("all_pairs",)) -> Workload:
+    """A workload of any size with the configurations' recipe: A from ``sampler``; B = ``n_copy`` perturbed copies of
+    random A sources + ``n_extra`` independent sources (used for the shapes of the paper's data sets, Table 2)."""
+    return _build(name, seed, int(n_a), int(n_copy), int(n_extra), sampler, sigma_arcsec, radius_arcsec, tuple(modes))
+
+
 def stress_classes(k_seed: int, n: int, grid: dict | None = None):
     """Class labels of config 4's A sources (same streams as ``config(4)``), for
     stratified subsampling.  Only valid for single-chunk sizes; larger callers

@@ -149,19 +149,21 @@ int hlc2_grid_describe(const hlc2_index* idx, hlc2_grid_info* info, const int32_
  *   x, y, z     [n] fp64 unit vectors in cell order      id  [n] int64 in cell order
  *   cell_start  [n_cells + 1] uint32, cell c holds sorted rows [cell_start[c], cell_start[c+1])
  *   cell_key    [n] uint32: the cell key of every sorted row in the low 28 bits (& HLC2_KEY_MASK); when the grid
- *               has <= 2^28 cells the top bits carry the row's window flags on its own grid (bit 28 / 29: a window of
- *               radius <= r_max reaches the previous / next RA cell of its zone; bit 30: it leaves the zone, passes
- *               RA = 0/360 or is wider than a cell), which let two indices on ONE grid (opts.grid_like) be matched
- *               without per-row window arithmetic.  With more cells the word is the bare key.
+ *               has <= 2^28 cells the top bits carry the row's window flags on its own grid -- bit 28 / 29: a window of
+ *               radius <= r_max reaches the previous / next RA cell of its zone; bit 30 / 31: it reaches the zone
+ *               below / above; both of 30 and 31: anything else (it passes RA = 0/360, is wider than a cell, or touches
+ *               both neighbouring zones: the general path) -- which let two indices on ONE grid (opts.grid_like) be
+ *               matched without per-row window arithmetic.  With more cells the word is the bare key.
  */
 #define HLC2_KEY_MASK 0x0FFFFFFFu
 int hlc2_index_arrays(const hlc2_index* idx, const double** d_x, const double** d_y, const double** d_z,
                       const int64_t** d_id, const uint32_t** d_cell_start, const uint32_t** d_cell_key,
                       int64_t* n, int64_t* n_cells);
 
-/* Scratch needed by hlc2_crossmatch for this pair of indices (may be 0): the job records into which the
- * planner cuts every A tile's window -- the role of the paper's calculation blocks, whose
- * memory the paper's tool sized itself (Eq. (8)-(9)) and the caller sizes here. */
+/* Scratch needed by hlc2_crossmatch / hlc2_selfmatch / hlc2_crossmatch_radii for this pair of indices (may be 0): for two
+ * indices on different grids the job records into which the planner cuts every A tile's window -- the role of the
+ * paper's calculation blocks, whose memory the paper's tool sized itself (Eq. (8)-(9)) and the
+ * caller sizes here; for two indices on one grid the list of the rows that need the general path (4 bytes per A row). */
 int hlc2_crossmatch_sizes(const hlc2_index* A, const hlc2_index* B, size_t* temp_bytes);
 
 /*

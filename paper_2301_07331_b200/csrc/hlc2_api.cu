@@ -494,6 +494,6 @@ int hlc2_last_cuda_error(const char** message) {
 
 unsigned long long hlc2_kernel_launches(void) { return hlc2::g_launches.load(std::memory_order_relaxed); }
 
-const char* hlc2_version(void) { return "hlc2-b200 0.2 (sm_100a)"; }
+const char* hlc2_version(void) { return "hlc2-b200 0.3 (sm_100a)"; }
 
 }  // extern "C"

@@ -274,17 +274,32 @@ k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
     }
     const unsigned lt = (1u << lane) - 1;
     uint32_t* mywh = wh + w * kRadix;
+    // ranks, six items at a time in three phases (all matches, then all counter bumps, then all broadcasts), so that the
+    // latencies of match_any, of the shared-memory atomics and of the shuffles overlap instead of adding up item by item
+    constexpr int kG = 6;
+    static_assert(kOsItems % kG == 0, "items are ranked in groups");
 #pragma unroll
-    for (int r = 0; r < kOsItems; ++r) {
-        const bool ok = base + (size_t)r * 32 < n;
-        const uint32_t d = ok ? ((k[r] >> shift) & mask) : 0xFFFFFFFFu;
-        const unsigned peers = __match_any_sync(0xffffffffu, d);
-        const uint32_t old = ok ? mywh[d] : 0u;
-        __syncwarp();
-        if (ok && (peers & lt) == 0) mywh[d] = old + (uint32_t)__popc(peers);
-        __syncwarp();
-        const uint32_t rank = old + (uint32_t)__popc(peers & lt);
-        if (r & 1) rk[r >> 1] |= rank << 16; else rk[r >> 1] = rank;
+    for (int g = 0; g < kOsItems; g += kG) {
+        uint32_t d[kG]; unsigned peers[kG]; uint32_t old[kG];
+#pragma unroll
+        for (int j = 0; j < kG; ++j) {
+            const bool ok = base + (size_t)(g + j) * 32 < n;
+            d[j] = ok ? ((k[g + j] >> shift) & mask) : 0xFFFFFFFFu;
+            peers[j] = __match_any_sync(0xffffffffu, d[j]);
+        }
+        // lanes with the same digit: the lowest of them bumps the warp's counter once for all and hands the old value
+        // round; the groups of one step are disjoint digits or the same counter in program order: atomics keep it exact
+#pragma unroll
+        for (int j = 0; j < kG; ++j) {
+            old[j] = 0;
+            if (d[j] != 0xFFFFFFFFu && lane == __ffs(peers[j]) - 1) old[j] = atomicAdd(&mywh[d[j]], (uint32_t)__popc(peers[j]));
+        }
+#pragma unroll
+        for (int j = 0; j < kG; ++j) {
+            const int r = g + j;
+            const uint32_t rank = __shfl_sync(0xffffffffu, old[j], __ffs(peers[j]) - 1) + (uint32_t)__popc(peers[j] & lt);
+            if (r & 1) rk[r >> 1] |= rank << 16; else rk[r >> 1] = rank;
+        }
     }
     __syncthreads();
 
@@ -299,13 +314,22 @@ k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
     const uint32_t loc = block_scan_incl(c, &tot, s_scan) - c;      // first position of digit d in the sorted tile
     uint32_t excl = 0;
     if (tile > 0) {
-        volatile uint32_t* p = my_status - kRadix;
-        for (;;) {
-            uint32_t sv = *p;
-            if ((sv & kFlagMask) == 0) continue;
-            excl += sv & ~kFlagMask;
-            if (sv & kFlagIncl) break;
-            p -= kRadix;
+        // look back over the predecessors' records, eight at a time (independent loads: one memory latency per eight
+        // tiles instead of one per tile); stop at the first inclusive prefix, re-poll from the first record not yet there
+        long long q = (long long)tile - 1;
+        for (bool done = false; !done;) {
+            uint32_t sv[8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) { sv[j] = 2u << 30; if (q - j >= 0) sv[j] = status[(size_t)(q - j) * kRadix + dgt]; }     // before tile 0: an empty inclusive prefix
+            int used = 8;
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                if (done || used != 8) continue;
+                if ((sv[j] & kFlagMask) == 0) { used = j; continue; }
+                excl += sv[j] & ~kFlagMask;
+                if (sv[j] & kFlagIncl) done = true;
+            }
+            q -= used;
         }
         *my_status = (excl + c) | kFlagIncl;
     }
