@@ -69,7 +69,7 @@ typedef enum {
  *                     Fine cells are never smaller than this ("cells sized to r", NS (a)), so a
  *                     search window spans at most 3 zones.
  *   target_occupancy  mean sources per fine cell over the occupied sky; 0 -> automatic: the finest value in
- *                     [0.5, 1] whose cell count needs no more radix-sort digits than occupancy 1 would.
+ *                     [0.4, 1] whose cell count needs no more radix-sort digits than occupancy 1 would.
  *   cell_arcsec       explicit fine-cell size; 0 -> derived from the catalogue's density
  *                     (max(r_max, sqrt(target_occupancy * occupied area / n))).  Honoured while the cell
  *                     table stays within max(16 n, 2^25) cells, else coarsened until it fits.
@@ -77,8 +77,9 @@ typedef enum {
  *   zone_aspect       zones are zone_aspect times as high as the fine-cell size and RA cells that much narrower (same
  *                     cell area, both never below r_max): a source's search window then leaves its zone zone_aspect times
  *                     less often and reaches a neighbouring RA cell that much more often -- the second is the cheap one
- *                     (one more cell of the same contiguous row range).  0 -> automatic: min(32, floor(cell / (3 r_max))), at
- *                     least 1; 1 = square cells.
+ *                     (one more cell of the same contiguous row range).  0 -> automatic: min(32, floor(cell / (3 r_max))), scaled
+ *                     back when the catalogue is concentrated in RA (fullest of 4096 RA bins more than 4x the mean
+ *                     occupied bin: a dense strip along a meridian would fill tall cells), at least 1; 1 = square cells.
  *   grid_like         if non-NULL, reuse that index's grid exactly (zones, cells, box).  The
  *                     catalogue must lie inside that grid's box (else HLC2_ERR_GRID_MISMATCH).
  */

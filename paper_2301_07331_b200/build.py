@@ -1,6 +1,6 @@
 """Build libhlc2.so (hand-written sm_100a CUDA + the C ABI of include/hlc2.h) in-tree with nvcc.
 
-    python -m paper_2301_07331_b200.build [--force]
+    python -m paper_2301_07331_b200.build [--force] [-v] [-DHLC2_DEBUG_BOUNDS]
 
 nvcc cross-compiles without a GPU.  The built library is git-ignored but travels with the tree.
 """
@@ -33,11 +33,12 @@ def needs_build() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and not needs_build():
+def build(force: bool = False, verbose: bool = False, defines=()) -> str:
+    """defines: extra -D macros (e.g. HLC2_DEBUG_BOUNDS: device-side index checks in the same-grid match kernel)."""
+    if not force and not defines and not needs_build():
         return SO
     tmp = SO + f".tmp{os.getpid()}"
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+    cmd = [_nvcc()] + NVCC_FLAGS + [f"-D{d}" for d in defines] + (["-Xptxas", "-v"] if verbose else []) + \
           ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.run(cmd, check=True)
     os.replace(tmp, SO)
@@ -45,4 +46,4 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, defines=[a[2:] for a in sys.argv[1:] if a.startswith("-D")]))

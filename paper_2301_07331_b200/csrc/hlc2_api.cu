@@ -71,13 +71,13 @@ static bool opts_ok(const hlc2_opts* o) {
 // target_occupancy 0 = automatic: cells as fine as the radix sort allows for free.  Finer cells of the scanned
 // catalogue mean fewer candidates per source in the match (config 3: occupancy 0.5 instead of 1 takes 7 % off the match),
 // but a cell count that needs one more key digit costs a whole extra sort pass in the build; so take the finest
-// occupancy in [0.5, 1] whose cell count still fits the digits that occupancy 1 needs.
+// occupancy in [0.4, 1] whose cell count still fits the digits that occupancy 1 needs.
 static double auto_occupancy(int64_t n) {
     if (n <= 0) return 1.0;
     int bits = 1; while (bits < 32 && (1ull << bits) < (unsigned long long)n) ++bits;      // key bits at occupancy 1
     const int passes = std::max(1, (bits + kRadixBits - 1) / kRadixBits);
     const double max_cells = std::ldexp(1.0, std::min(32, passes * kRadixBits));
-    return std::min(1.0, std::max(0.5, 1.15 * (double)n / max_cells));
+    return std::min(1.0, std::max(0.4, 1.15 * (double)n / max_cells));
 }
 static hlc2_opts opts_or_default(const hlc2_opts* o, int64_t n) {
     hlc2_opts d; memset(&d, 0, sizeof d); d.r_max_arcsec = 1.0;
@@ -203,11 +203,24 @@ static void plan_grid(const Stats& st, int64_t n_valid, const hlc2_opts& o, size
     }
     c = std::max(c, o.r_max_arcsec);
     c = std::min(c, 648000.0);
+    double ra_contrast = 1.0;
+    if (n_valid > 0) {
+        uint64_t occ = 0, mx = 0;
+        for (int i = 0; i < kRaBins; ++i) { if (st.ra_hist[i]) ++occ; mx = std::max<uint64_t>(mx, st.ra_hist[i]); }
+        if (occ) ra_contrast = (double)mx * (double)occ / (double)n_valid;
+    }
     for (int iter = 0; iter < 2000; ++iter) {
         // zones `aspect` times as high as the cell size, RA cells that much narrower (never below r_max): same cell area,
         // but a search window leaves its zone (the expensive neighbour) aspect times less often
-        // automatic: RA cells three r_max wide (measured on config 3: the match time falls until about there)
-        const double want = o.zone_aspect > 0 ? (double)o.zone_aspect : std::min(32.0, floor(c / (3.0 * o.r_max_arcsec)));
+        // automatic: RA cells three r_max wide (measured on config 3: the match time falls until about there) -- unless the
+        // catalogue is concentrated in RA (a dense strip along a meridian, config 4's seam): tall cells would then hold
+        // the whole strip's height.  The coarse RA histogram of the extent pass tells: contrast = fullest bin / mean
+        // occupied bin; beyond 4 the aspect is scaled back in proportion (config 3: 1.3 -> 24; config 4: 200 -> 1).
+        double want = (double)o.zone_aspect;
+        if (o.zone_aspect <= 0) {
+            want = std::min(32.0, floor(c / (3.0 * o.r_max_arcsec)));
+            if (ra_contrast > 4.0) want = floor(want * 4.0 / ra_contrast);
+        }
         const double aspect = std::max(1.0, std::min(want, c / o.r_max_arcsec));
         double zh_deg = std::min(c * aspect, 648000.0) / 3600.0;
         double rng = std::max(range, zh_deg);

@@ -24,9 +24,19 @@
 //     Rows flagged kKeyGeneral (window through RA = 0/360, polar rows) are set aside and take the general per-lane path.
 //
 // Decisions are fp64; the flags only ever select a superset of cells.
+#include <assert.h>
+
 #include <algorithm>
 
 #include "hlc2_match_common.cuh"
+
+// -DHLC2_DEBUG_BOUNDS: device-side checks of every shared-memory index the kernel computes (compute-sanitizer is
+// closed on the B200 pool; the GPU tests are run once per round against a library built this way)
+#ifdef HLC2_DEBUG_BOUNDS
+#define HLC2_CHECK(c) assert(c)
+#else
+#define HLC2_CHECK(c) ((void)0)
+#endif
 
 namespace hlc2 {
 
@@ -151,6 +161,7 @@ __device__ __forceinline__ void ring_push(const IndexView& A, const IndexView& B
         ring_drain_rows(A, B, p, w, os.head, os.tail, os.pend, os.base0, os.base1, lane);
         os.head = os.tail; os.pend = 0;
     }
+    HLC2_CHECK(os.tail - os.head + __popc(m) <= (unsigned)kRing);
     if (hit) {
         const unsigned e = (os.tail + __popc(m & ((1u << lane) - 1u))) & (kRing - 1);
         w.qa[e] = a_row; w.qb[e] = b_row; w.qc2[e] = c2;
@@ -188,7 +199,9 @@ k_match_general_rows(const __grid_constant__ IndexView A, const __grid_constant_
     }
 }
 
-template <int MODE>
+// SELF: the catalogue is matched with itself (p.self_mode != 0); a template switch so that the ordinary match does not
+// pay for the filters in its candidate loop
+template <int MODE, bool SELF>
 __global__ void __launch_bounds__(kMatchThreads, HLC2_SCTAS)
 k_match_same(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B, const __grid_constant__ MatchArgs p,
              uint32_t* __restrict__ glist, uint32_t* __restrict__ glist_count) {
@@ -276,6 +289,7 @@ k_match_same(const __grid_constant__ IndexView A, const __grid_constant__ IndexV
                 const uint32_t a_al = a_first & ~1u, k_al = a_first & ~3u;
                 const uint32_t a_ld = first ? ((a_first + a_count + 1u) & ~1u) - a_al : 0u, k_ld = first ? ((a_first + a_count + 3u) & ~3u) - k_al : 0u;
                 const uint32_t bytes = n_ld * 24u + c_ld * 4u + a_ld * 24u + k_ld * 4u;
+                HLC2_CHECK(n_ld <= (uint32_t)kSBCap && c_ld <= (uint32_t)kSCsCap && a_ld <= (uint32_t)kTile + 2u && k_ld <= (uint32_t)kTile + 4u);
                 if (lane == 0) {
                     uint4* d = reinterpret_cast<uint4*>(&st.d);
                     d[0] = make_uint4(flags, cs_al, row_al, r); d[1] = make_uint4(re, (uint32_t)nn, a_first, a_count);
@@ -346,6 +360,7 @@ k_match_same(const __grid_constant__ IndexView A, const __grid_constant__ IndexV
         const uint32_t a_row = dw.z + threadIdx.x;
         if (flags & kSFirst) {            // a new tile: its rows came with this stage
             const unsigned ra = (mine ? threadIdx.x : 0u) + st.d.a_off;
+            HLC2_CHECK(ra < (unsigned)kTile + 2u && (mine ? threadIdx.x : 0u) + st.d.k_off < (unsigned)kTile + 4u);
             ax = st.ax[ra]; ay = st.ay[ra]; az = st.az[ra]; kf = st.ak[(mine ? threadIdx.x : 0u) + st.d.k_off];
             best.has = false;
             const bool gen = mine && (kf >> 30) == 3u;
@@ -365,10 +380,10 @@ k_match_same(const __grid_constant__ IndexView A, const __grid_constant__ IndexV
         uint32_t self_lo = 0;              // self-match, every unordered pair once: only B rows behind the A row count
         if ((flags & (kSLo | kSHi)) == 0u) {
             c0 = key - (uint32_t)elo; c1 = key + (uint32_t)ehi;
-            if (p.self_mode == 1) self_lo = a_row + 1u; else if (p.self_mode == 2) self_lo = a_row;
+            if (SELF) { if (p.self_mode == 1) self_lo = a_row + 1u; else if (p.self_mode == 2) self_lo = a_row; }
         } else {
             act = act && (kf & ((flags & kSLo) ? kKeyDecLo : kKeyDecHi)) != 0u;
-            if ((flags & kSLo) && (p.self_mode == 1 || p.self_mode == 2)) act = false;      // the zone below holds earlier rows only
+            if (SELF && (flags & kSLo) && (p.self_mode == 1 || p.self_mode == 2)) act = false;      // the zone below holds earlier rows only
             const int k = (int)(key - st.d.cb_own);
             c0 = st.d.cb_nb + (uint32_t)nb_first(k - elo, st.d.c_lo); c1 = st.d.cb_nb + (uint32_t)nb_last(k + ehi, (int)dw.y, st.d.c_hi);
         }
@@ -378,9 +393,11 @@ k_match_same(const __grid_constant__ IndexView A, const __grid_constant__ IndexV
         } else {
             unsigned p0 = 0, len = 0;
             if (act) {
+                HLC2_CHECK(c0 >= dv.y && c0 <= c1 && c1 + 1u - dv.y < (uint32_t)kSCsCap);
                 const uint32_t q1 = min(max(st.cs[c1 + 1u - dv.y], dv.w), dw.x);
-                const uint32_t q0 = min(max(max(st.cs[c0 - dv.y], dv.w), self_lo), q1);
+                const uint32_t q0 = SELF ? min(max(max(st.cs[c0 - dv.y], dv.w), self_lo), q1) : min(max(st.cs[c0 - dv.y], dv.w), dw.x);
                 p0 = q0 - dv.z; len = q1 - q0;
+                HLC2_CHECK(q0 >= dv.z && q1 - dv.z <= (uint32_t)kSBCap);
             }
             const unsigned mx = __reduce_max_sync(kFull, len);
             // a lane past its own range keeps reading on (rows of other lanes, at worst the arrays behind bx: all inside
@@ -391,7 +408,7 @@ k_match_same(const __grid_constant__ IndexView A, const __grid_constant__ IndexV
                 const double dx = ax - st.bx[j], dy = ay - st.by[j], dz = az - st.bz[j];
                 const double c2v = fma(dx, dx, fma(dy, dy, dz * dz));
                 const uint32_t r = j + dv.z;
-                const bool hit = in && c2v <= p.thr2 && (p.self_mode != 3 || r != a_row);
+                const bool hit = in && c2v <= p.thr2 && (!SELF || p.self_mode != 3 || r != a_row);
                 if (hit) {
                     if (MODE == HLC2_ALL_PAIRS) {
                         // a lane holds its first pair of the tile (queued with everybody's at the tile's end: one ballot per
@@ -441,22 +458,25 @@ size_t match_same_temp_bytes(const IndexView& A) { return 256 + (size_t)A.n * si
 void launch_match_same(const IndexView& A, const IndexView& B, const MatchArgs& p, int mode, void* d_temp, cudaStream_t s,
                        cudaEvent_t ev_start, cudaEvent_t ev_stop) {
     const int m = mode == HLC2_NEAREST ? 1 : 0;
-    const void* kern = m == 0 ? (const void*)k_match_same<HLC2_ALL_PAIRS> : (const void*)k_match_same<HLC2_NEAREST>;
-    static int per_sm_dev[kMaxDevices][2] = {};        // resident CTAs per SM; the smem opt-in is per device
+    const bool self = p.self_mode != 0;
+    const void* kern = self ? (m == 0 ? (const void*)k_match_same<HLC2_ALL_PAIRS, true> : (const void*)k_match_same<HLC2_NEAREST, true>)
+                            : (m == 0 ? (const void*)k_match_same<HLC2_ALL_PAIRS, false> : (const void*)k_match_same<HLC2_NEAREST, false>);
+    static int per_sm_dev[kMaxDevices][4] = {};        // resident CTAs per SM; the smem opt-in is per device
     int* per_sm = per_sm_dev[current_device()];
     const size_t smem = sizeof(SSmem);
-    if (!per_sm[m]) {
+    const int mi = m + (self ? 2 : 0);
+    if (!per_sm[mi]) {
         int v = 0;
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         cudaOccupancyMaxActiveBlocksPerMultiprocessor(&v, kern, kMatchThreads, smem);
-        per_sm[m] = v > 0 ? v : 1;
+        per_sm[mi] = v > 0 ? v : 1;
     }
     // scratch: 256-byte header (count of general rows), then their row numbers
     uint32_t* glist_count = reinterpret_cast<uint32_t*>(d_temp);
     uint32_t* glist = reinterpret_cast<uint32_t*>(reinterpret_cast<char*>(d_temp) + 256);
     cudaMemsetAsync(glist_count, 0, sizeof(uint32_t), s);
     // persistent grid: SM count x resident CTAs, never more CTAs than tiles
-    const unsigned blocks = (unsigned)std::max<size_t>(1, std::min<size_t>(A.tile_cap, (size_t)sm_count() * per_sm[m]));
+    const unsigned blocks = (unsigned)std::max<size_t>(1, std::min<size_t>(A.tile_cap, (size_t)sm_count() * per_sm[mi]));
     if (ev_start) cudaEventRecord(ev_start, s);          // the caller's events bracket the match kernels (hlc2_crossmatch_events)
     void* kargs[5] = {(void*)&A, (void*)&B, (void*)&p, (void*)&glist, (void*)&glist_count};
     cudaLaunchKernel(kern, dim3(blocks), dim3(kMatchThreads), kargs, smem, s);
