@@ -68,18 +68,6 @@ __device__ __forceinline__ void mbar_wait(unsigned long long* b, unsigned parity
                      : "=r"(done) : "r"(a), "r"(parity), "r"(0x4000u) : "memory");
     } while (!done);
 }
-// the same for a waiter with slack (the producer, several stages ahead): sleep between polls, so that the retry loop
-// does not take issue slots from the warps doing the arithmetic
-__device__ __forceinline__ void mbar_wait_relaxed(unsigned long long* b, unsigned parity) {
-    const uint32_t a = smem_u32(b);
-    for (;;) {
-        unsigned done;
-        asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
-                     : "=r"(done) : "r"(a), "r"(parity) : "memory");
-        if (done) break;
-        __nanosleep(400);
-    }
-}
 // global -> shared bulk copy, completion counted in bytes on an mbarrier; 16-byte aligned src, dst and size
 __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* b) {
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"

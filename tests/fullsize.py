@@ -128,7 +128,10 @@ def cfg4_workload(P, scale=1.0):
     the grid comes from hlc2_grid_describe of a preliminary index built with the same options."""
     import torch
     n_b = int(round(20_000_000 * scale))
-    opts = P.make_opts(3.0, cell_arcsec=160.0, full_sky=True)
+    # config 4's nominal grid: square 160-arcsec cells over the full sky (the stress mix has a dense strip along the RA = 0
+    # meridian: cells taller than wide would each hold a long piece of it; an index planned from the stress catalogue itself
+    # sees that in its RA histogram and keeps its cells square, this preliminary one is planned from uniform points)
+    opts = P.make_opts(3.0, cell_arcsec=160.0, full_sky=True, zone_aspect=1)
     ra, dec = S.uniform_sphere(np.random.default_rng(1), min(n_b, 1_000_000))
     pre = P.hlc2_build_index(torch.from_numpy(ra).cuda(), torch.from_numpy(dec).cuda(), None, opts=opts)
     grid = P.hlc2_grid_describe(pre)
@@ -153,7 +156,7 @@ def report(P, cfg, scale=1.0, one_core=False, same_grid=False, out_dir=None, bru
     like_b = None; grid = None
     if cfg == 4:
         w, like_b, grid = cfg4_workload(P, scale)
-        opts_a = P.make_opts(3.0, cell_arcsec=160.0, full_sky=True); opts_b = P.make_opts(3.0)
+        opts_a = P.make_opts(3.0, cell_arcsec=160.0, full_sky=True, zone_aspect=1); opts_b = P.make_opts(3.0)
         if same_grid:
             opts_a = P.make_opts(3.0)
     else:

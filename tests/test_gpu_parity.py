@@ -130,12 +130,12 @@ def test_cfg4_boundary_stress_vs_brute_force(P):
     import torch
     scale = 0.01                                                     # 2e5 x 2e5, r = 3 arcsec
     n_b = int(round(20_000_000 * scale))
-    opts = P.make_opts(3.0, cell_arcsec=160.0, full_sky=True)        # config 4's nominal grid: 160" cells, full sky
+    opts = P.make_opts(3.0, cell_arcsec=160.0, full_sky=True, zone_aspect=1)   # config 4's nominal grid: square 160" cells, full sky
     prelim_ra, prelim_dec = S.uniform_sphere(np.random.default_rng(1), n_b)
     pre = P.hlc2_build_index(torch.from_numpy(prelim_ra).cuda(), torch.from_numpy(prelim_dec).cuda(), None, opts=opts)
     grid = P.hlc2_grid_describe(pre)
     w = S.config(4, scale=scale, grid=grid)
-    ia = P.hlc2_build_index(*dev(w.A), opts=P.make_opts(3.0, cell_arcsec=160.0, full_sky=True))
+    ia = P.hlc2_build_index(*dev(w.A), opts=P.make_opts(3.0, cell_arcsec=160.0, full_sky=True, zone_aspect=1))
     ib = P.hlc2_build_index(*dev(w.B), opts=P.make_opts(3.0), like=pre)          # exactly the described grid
     gb_grid = P.hlc2_grid_describe(ib)
     assert gb_grid["n_cells"] == grid["n_cells"] and np.array_equal(gb_grid["n_ra"], grid["n_ra"])
