@@ -149,18 +149,28 @@ def stratified_subsample(w, grid, m=200_000, seed=4):
     return np.sort(np.concatenate(rows))
 
 
+# The workload and the oracle's rows of a configuration are computed once per process: the two-grid and the same-grid run of
+# a configuration compare against the same expected rows (the oracle on config 3 alone is 45 s of the box's 16 cores).
+_workloads = {}
+_expected = {}
+
+
 def report(P, cfg, scale=1.0, one_core=False, same_grid=False, out_dir=None, brute_rows=200_000):
     """Run configuration `cfg` at `scale` (1.0 = the stated size) and compare every mode with the oracle."""
     import torch
     t0 = time.perf_counter()
     like_b = None; grid = None
     if cfg == 4:
-        w, like_b, grid = cfg4_workload(P, scale)
+        if (cfg, scale) not in _workloads:
+            _workloads[(cfg, scale)] = cfg4_workload(P, scale)
+        w, like_b, grid = _workloads[(cfg, scale)]
         opts_a = P.make_opts(3.0, cell_arcsec=160.0, full_sky=True, zone_aspect=1); opts_b = P.make_opts(3.0)
         if same_grid:
             opts_a = P.make_opts(3.0)
     else:
-        w = S.config(cfg, scale=scale)
+        if (cfg, scale) not in _workloads:
+            _workloads[(cfg, scale)] = S.config(cfg, scale=scale)
+        w = _workloads[(cfg, scale)]
         opts_a = opts_b = P.make_opts(w.radius_arcsec)
     t_gen = time.perf_counter() - t0
     r = w.radius_arcsec
@@ -172,10 +182,12 @@ def report(P, cfg, scale=1.0, one_core=False, same_grid=False, out_dir=None, bru
         gk, gs = gpu_rows_sorted(a, b, s)
         del a, b, s
         torch.cuda.empty_cache()
-        t1 = time.perf_counter()
-        oa, ob, osep, used = oracle.match(w.A.ra, w.A.dec, w.A.id, w.B.ra, w.B.dec, w.B.id, r, mode)
-        t_or = time.perf_counter() - t1
-        ok = pack(oa, ob)
+        if (cfg, scale, mode) not in _expected:
+            t1 = time.perf_counter()
+            oa, ob, osep, used = oracle.match(w.A.ra, w.A.dec, w.A.id, w.B.ra, w.B.dec, w.B.id, r, mode)
+            _expected[(cfg, scale, mode)] = (pack(oa, ob), osep, used, time.perf_counter() - t1)
+            del oa, ob
+        ok, osep, used, t_or = _expected[(cfg, scale, mode)]
         rep = compare_packed(gk, gs, ok, osep, r, w.A, w.B, nearest=mode == P.HLC2_NEAREST)
         rep.update(t_build_a_ms=tm["build_a"], t_build_b_ms=tm["build_b"], t_match_ms=tm["match"],
                    a_src_per_s_match=len(w.A) / (tm["match"] * 1e-3), pairs_per_s_match=len(gk) / (tm["match"] * 1e-3),
@@ -189,11 +201,12 @@ def report(P, cfg, scale=1.0, one_core=False, same_grid=False, out_dir=None, bru
         if cfg == 4 and mode == P.HLC2_ALL_PAIRS:
             # the prescribed completeness check: brute force ("No Index") on a stratified subsample of A
             rows = stratified_subsample(w, grid, min(brute_rows, len(w.A)))
-            sub = w.A.take(rows)
-            t1 = time.perf_counter()
-            ba, bb, bs, _ = oracle.match(sub.ra, sub.dec, sub.id, w.B.ra, w.B.dec, w.B.id, r, mode, oracle.ENGINE_BRUTE)
-            t_bf = time.perf_counter() - t1
-            bk = pack(ba, bb)
+            if (cfg, scale, "brute", len(rows)) not in _expected:
+                sub = w.A.take(rows)
+                t1 = time.perf_counter()
+                ba, bb, bs, _ = oracle.match(sub.ra, sub.dec, sub.id, w.B.ra, w.B.dec, w.B.id, r, mode, oracle.ENGINE_BRUTE)
+                _expected[(cfg, scale, "brute", len(rows))] = (pack(ba, bb), bs, time.perf_counter() - t1)
+            bk, bs, t_bf = _expected[(cfg, scale, "brute", len(rows))]
             sel = np.isin(gk >> 31, rows)
             brep = compare_packed(gk[sel], gs[sel], bk, bs, r, w.A, w.B)
             rep["brute_force_subsample"] = dict(rows=int(len(rows)), seconds=t_bf, **brep)
