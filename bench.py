@@ -446,7 +446,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--occupancy", type=float, default=0.0)
     ap.add_argument("--occupancy-b", type=float, default=None, help="target occupancy of B's index (default: same as --occupancy)")
-    ap.add_argument("--bands", type=int, default=16, help="declination bands of the streamed e2e leg")
+    ap.add_argument("--bands", type=int, default=0, help="declination bands of the streamed legs (0: 32 for the e2e leg of a resident configuration -- measured best of 16 / 32 / 64 on config 3 -- and 64 for --config 5)")
     ap.add_argument("--no-stream", action="store_true", help="skip the streamed e2e leg")
     ap.add_argument("--shape", default=None, choices=["D2", "D4", "D6"], help="end to end at the shape of one of the paper's data sets (Table 2) instead of a configuration")
     args = ap.parse_args()
@@ -463,7 +463,7 @@ def main():
         torch.cuda.set_device(local_rank)
         if args.shape:
             return run_shape(args, local_rank)
-        if args.bands == 16: args.bands = 64
+        if args.bands <= 0: args.bands = 64
         return run_config5(args, local_rank)
     t0 = time.perf_counter()
     # replicas: every rank generates its own catalogue (different seed) of the same shape
@@ -586,7 +586,7 @@ def main():
     # hlc2_stream_crossmatch per step: H2D of band k+1, build + match of band k and D2H of band k-1 overlap ----
     t_stream_ms, stream_info = None, None
     if not args.no_stream:
-        nb = args.bands
+        nb = args.bands if args.bands > 0 else 32
         edges = np.quantile(w.A.dec[:: max(1, n_a // 2_000_000)], np.linspace(0.0, 1.0, nb + 1))
         edges[0], edges[-1] = -90.0, 90.0
         Ab, a_off = S.to_bands(w.A, edges); Bb, b_off = S.to_bands(w.B, edges)
