@@ -113,3 +113,23 @@ def test_cfg5_streamed_nearest_scaled(P):
     oa, ob, os_, _ = oracle.match(w.A.ra, w.A.dec, w.A.id, w.B.ra, w.B.dec, w.B.id, w.radius_arcsec, 1)
     rep = parity.compare_nearest((ga, gb, gs), (oa, ob, os_), w.radius_arcsec, parity.make_sep_of(w.A, w.B))
     assert rep["n_gpu"] > 50_000
+
+
+def test_bench_streamed_legs_emit_the_contract_line():
+    """bench.py --config 5 (at a stated small scale) and --shape D2: one JSON line each with the contract's keys, the PCIe
+    roofline, the oracle check of the sampled bands and the fitted cost model."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    for extra in (["--config", "5", "--scale", "0.002", "--bands", "16"], ["--shape", "D2"]):
+        out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--steps", "1", "--warmup", "1"] + extra,
+                             capture_output=True, text=True, timeout=600, cwd=root)
+        assert out.returncode == 0, out.stderr[-2000:]
+        line = json.loads(out.stdout.strip().splitlines()[-1])
+        for key in ("metric", "value", "unit", "n_gpus", "ms_per_step", "config", "e2e", "roofline", "cpu_baseline", "verify", "model", "gpu_launches"):
+            assert key in line, key
+        assert line["roofline"]["bound"] == "pcie" and 0.0 < line["roofline"]["frac"] < 1.2
+        assert line["verify"]["rows_gpu"] == line["verify"]["rows_oracle"] > 1000 and line["gpu_launches"] > 0
+        assert line["model"]["eq6_sum_ms"] >= line["model"]["overlapped_max_ms"] > 0.0
