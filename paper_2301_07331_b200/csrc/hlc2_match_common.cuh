@@ -103,10 +103,13 @@ __device__ __forceinline__ void emit_direct(const IndexView& A, const IndexView&
 
 template <int MODE>
 __device__ __forceinline__ void scan_global(const IndexView& A, const IndexView& B, const MatchArgs& p, uint32_t a_row,
-                                            double ax, double ay, double az, uint32_t j0, uint32_t j1, Best& h) {
+                                            double ax, double ay, double az, uint32_t j0, uint32_t j1, Best& h,
+                                            uint32_t off = 0, uint32_t stride = 1) {
+    // (off, stride) = (0, 1): the calling lane walks the whole range; (lane, 32): a warp shares one A row and its lanes
+    // take every 32nd candidate (coalesced loads: the way to walk long ranges, e.g. dense cells at the RA seam)
     if (p.self_mode == 1) j0 = max(j0, a_row + 1u); else if (p.self_mode == 2) j0 = max(j0, a_row);
     const double ea2 = p.eb2 ? __ldg(p.ea2 + a_row) : 0.0;
-    for (uint32_t j = j0; j < j1; ++j) {
+    for (uint32_t j = j0 + off; j < j1; j += stride) {
         if (p.self_mode == 3 && j == a_row) continue;
         const double dx = ax - __ldg(B.x + j), dy = ay - __ldg(B.y + j), dz = az - __ldg(B.z + j);
         const double c2 = fma(dx, dx, fma(dy, dy, dz * dz));
@@ -120,7 +123,8 @@ __device__ __forceinline__ void scan_global(const IndexView& A, const IndexView&
 
 template <int MODE>
 __device__ __noinline__ void scan_general(const IndexView& A, const IndexView& B, const MatchArgs& p, uint32_t a_row,
-                                          double ax, double ay, double az, float2 pf, Best& h) {
+                                          double ax, double ay, double az, float2 pf, Best& h,
+                                          uint32_t off = 0, uint32_t stride = 1) {
     const GridView& g = B.g;
     const double dlo = (double)pf.y - p.pad_dec, dhi = (double)pf.y + p.pad_dec;
     if (!(dhi >= g.dec_min && dlo <= g.dec_max)) return;          // also rows with a bad coordinate (NaN vector)
@@ -145,9 +149,9 @@ __device__ __noinline__ void scan_general(const IndexView& A, const IndexView& B
             if (!va) { if (!vx) continue; k0 = k2; k1 = k3; vx = false; }
             if (!vx) k3 = k2 - 1;
         }
-        scan_global<MODE>(A, B, p, a_row, ax, ay, az, __ldg(B.cell_start + base + k0), __ldg(B.cell_start + base + k1 + 1), h);
+        scan_global<MODE>(A, B, p, a_row, ax, ay, az, __ldg(B.cell_start + base + k0), __ldg(B.cell_start + base + k1 + 1), h, off, stride);
         if (k3 >= k2)
-            scan_global<MODE>(A, B, p, a_row, ax, ay, az, __ldg(B.cell_start + base + k2), __ldg(B.cell_start + base + k3 + 1), h);
+            scan_global<MODE>(A, B, p, a_row, ax, ay, az, __ldg(B.cell_start + base + k2), __ldg(B.cell_start + base + k3 + 1), h, off, stride);
     }
 }
 

@@ -185,17 +185,29 @@ __device__ __forceinline__ void ring_step(const IndexView& A, const IndexView& B
 }
 
 // Rows flagged kKeyGeneral (window through RA = 0/360, polar rows): k_match_same appends them to a list in the caller's
-// scratch (no calls inside its consumer loop), this kernel gives each one lane and the general per-lane path.
+// scratch (no calls inside its consumer loop), this kernel walks the general path for each of them with a whole warp:
+// the lanes share the row's window and take every 32nd candidate, so that the long row ranges such rows tend to have
+// (a dense strip along the RA = 0 meridian, a polar cap) are read with coalesced loads instead of lane by lane.
 template <int MODE>
 __global__ void __launch_bounds__(256)
 k_match_general_rows(const __grid_constant__ IndexView A, const __grid_constant__ IndexView B, const __grid_constant__ MatchArgs p,
                      const uint32_t* __restrict__ list, const uint32_t* __restrict__ list_count) {
     const uint32_t n = __ldg(list_count);
-    for (uint32_t i = blockIdx.x * 256 + threadIdx.x; i < n; i += gridDim.x * 256) {
+    const uint32_t lane = threadIdx.x & 31u;
+    for (uint32_t i = blockIdx.x * 8 + (threadIdx.x >> 5); i < n; i += gridDim.x * 8) {
         const uint32_t row = __ldg(list + i);
         Best h; h.has = false; h.c2 = 0.0; h.row = 0;
-        scan_general<MODE>(A, B, p, row, __ldg(A.x + row), __ldg(A.y + row), __ldg(A.z + row), __ldg(A.pos + row), h);
-        if (MODE == HLC2_NEAREST && h.has) emit_direct(A, B, p, row, h.row, h.c2);
+        scan_general<MODE>(A, B, p, row, __ldg(A.x + row), __ldg(A.y + row), __ldg(A.z + row), __ldg(A.pos + row), h, lane, 32u);
+        __syncwarp();
+        if (MODE == HLC2_NEAREST) {          // the nearest of the lanes' nearest; ties -> smaller idB
+            double c = h.has ? h.c2 : 1e300;
+            for (int o = 16; o; o >>= 1) c = fmin(c, __shfl_xor_sync(kFull, c, o));
+            const bool cand = h.has && h.c2 == c;
+            long long v = cand ? (long long)__ldg(B.id + h.row) : 0x7fffffffffffffffll;
+            for (int o = 16; o; o >>= 1) v = min(v, __shfl_xor_sync(kFull, v, o));
+            const unsigned m = __ballot_sync(kFull, cand && (long long)__ldg(B.id + h.row) == v);
+            if (m && (int)lane == __ffs(m) - 1) emit_direct(A, B, p, row, h.row, h.c2);
+        }
     }
 }
 
