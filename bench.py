@@ -505,7 +505,8 @@ def main():
     buf_a = torch.empty(ib_a, dtype=torch.uint8, device="cuda")
     if tb_a > tb_b:
         temp = torch.empty(tb_a, dtype=torch.uint8, device="cuda")
-    cap = int(max(n_a, n_b) * 0.5) + 1024 if mode == 0 else n_a
+    # output rows: config 3 finds 0.3 per A source; the others up to 2.2 per source (config 4's dense strips and caps)
+    cap = (int(max(n_a, n_b) * (0.5 if args.config == 3 else 2.5)) + 1024) if mode == 0 else n_a
     out_a = torch.empty(cap, dtype=torch.int64, device="cuda"); out_b = torch.empty(cap, dtype=torch.int64, device="cuda")
     out_s = torch.empty(cap, dtype=torch.float64, device="cuda"); cnt = torch.zeros(1, dtype=torch.int64, device="cuda")
     h_out = [torch.empty(cap, dtype=torch.int64).pin_memory(), torch.empty(cap, dtype=torch.int64).pin_memory(),
