@@ -492,7 +492,8 @@ def main():
     dA = [t.cuda(non_blocking=True) for t in hA]; dB = [t.cuda(non_blocking=True) for t in hB]
     torch.cuda.synchronize()
 
-    opts_a = P.make_opts(r, target_occupancy=args.occupancy); opts_b = P.make_opts(r, target_occupancy=args.occupancy if args.occupancy_b is None else args.occupancy_b)
+    # shared grid: A is filed on B's grid, which needs no extent pass and no host synchronisation (opts.async_like)
+    opts_a = P.make_opts(r, target_occupancy=args.occupancy, async_like=args.grid == "shared"); opts_b = P.make_opts(r, target_occupancy=args.occupancy if args.occupancy_b is None else args.occupancy_b)
     ib_b, tb_b = P.hlc2_index_sizes(n_b, opts_b)
     buf_b = torch.empty(ib_b, dtype=torch.uint8, device="cuda")
     temp = torch.empty(tb_b, dtype=torch.uint8, device="cuda")
@@ -536,6 +537,7 @@ def main():
     torch.cuda.synchronize()
     found = int(cnt.item())
     assert found <= cap, f"output capacity {cap} too small for {found} rows"
+    assert P.hlc2_index_status(ia)[0] == 0 and P.hlc2_index_status(ib)[0] == 0, "index status"
     grid_a, grid_b = P.hlc2_grid_describe(ia), P.hlc2_grid_describe(ib)
 
     # ---- timed region 1: inputs resident in HBM (inputs 3.6 GB >> 126 MB L2, so every step starts cold) ----

@@ -29,7 +29,7 @@
  *     only small host-side metadata; release it with hlc2_index_destroy.
  *   - Stream order: all device work is enqueued on `cuda_stream` (a cudaStream_t passed as
  *     void*; NULL = the legacy default stream).  hlc2_build_index synchronises that stream
- *     once (it reads back the catalogue extent to plan the grid); hlc2_crossmatch does not
+ *     once (it reads back the catalogue extent to plan the grid) unless opts.async_like is set; hlc2_crossmatch does not
  *     synchronise; hlc2_index_status synchronises.
  *   - Every function returns an int status: HLC2_OK (0) or a negative hlc2_status code.
  *   - n = 0 is valid everywhere and yields an empty result.
@@ -92,6 +92,12 @@ typedef struct {
     const hlc2_index* grid_like;
     const double* d_err_arcsec;      /* optional: [n] per-record error radii (device, input order, arcsec, >= 0) for
                                         hlc2_crossmatch_radii: the r1 / r2 of Eq. (4); NULL = none */
+    int32_t async_like;              /* with grid_like: build WITHOUT the extent pass and without any host synchronisation
+                                        (everything is enqueued on the stream; the call can be captured in a CUDA graph).
+                                        Bad coordinates and a catalogue that does not fit the grid's RA box are then both
+                                        reported by hlc2_index_status (HLC2_ERR_BAD_COORD / HLC2_ERR_GRID_MISMATCH), not by
+                                        the build call; sources outside the box are filed in the box's last cell. */
+    int32_t reserved;
 } hlc2_opts;
 
 /* Description of an index's grid (host data), for tools and for the boundary-stress generator. */

@@ -47,7 +47,8 @@ class Hlc2Error(RuntimeError):
 class hlc2_opts(ctypes.Structure):
     _fields_ = [("r_max_arcsec", ctypes.c_double), ("target_occupancy", ctypes.c_double),
                 ("cell_arcsec", ctypes.c_double), ("full_sky", ctypes.c_int32), ("zone_aspect", ctypes.c_int32),
-                ("grid_like", ctypes.c_void_p), ("d_err_arcsec", ctypes.c_void_p)]
+                ("grid_like", ctypes.c_void_p), ("d_err_arcsec", ctypes.c_void_p),
+                ("async_like", ctypes.c_int32), ("reserved", ctypes.c_int32)]
 
 
 class hlc2_grid_info(ctypes.Structure):
@@ -103,12 +104,14 @@ def _stream_ptr(stream):
     return ctypes.c_void_p(s.cuda_stream)
 
 
-def make_opts(r_max_arcsec=1.0, target_occupancy=0.0, cell_arcsec=0.0, full_sky=False, grid_like=None, zone_aspect=0) -> hlc2_opts:
+def make_opts(r_max_arcsec=1.0, target_occupancy=0.0, cell_arcsec=0.0, full_sky=False, grid_like=None, zone_aspect=0,
+              async_like=False) -> hlc2_opts:
     o = hlc2_opts()
     o.r_max_arcsec = float(r_max_arcsec); o.target_occupancy = float(target_occupancy)
     o.cell_arcsec = float(cell_arcsec); o.full_sky = int(bool(full_sky)); o.zone_aspect = int(zone_aspect)
     o.grid_like = grid_like.handle if grid_like is not None else None
     o.d_err_arcsec = None
+    o.async_like = int(bool(async_like)); o.reserved = 0
     return o
 
 
@@ -176,7 +179,7 @@ def hlc2_build_index(ra_deg, dec_deg, ids=None, opts: hlc2_opts | None = None, s
 def hlc2_index_status(idx: Index):
     row = ctypes.c_int64(-1)
     rc = lib().hlc2_index_status(idx.handle, ctypes.byref(row))
-    if rc not in (HLC2_OK, HLC2_ERR_BAD_COORD):
+    if rc not in (HLC2_OK, HLC2_ERR_BAD_COORD, HLC2_ERR_GRID_MISMATCH):
         raise Hlc2Error(rc, "hlc2_index_status")
     return rc, row.value
 

@@ -55,6 +55,8 @@ struct hlc2_index {
     int device;
     Stats h_stats;        // copy of the extent pass
     bool stats_valid;
+    Stats* d_stats;       // device copy of the status record (read lazily after an asynchronous build)
+    bool outside_box;     // asynchronous build: some source lies outside the grid's RA box
     bool flagged;         // the sorted keys carry window flags in their top bits (grids of <= 2^28 cells)
 };
 static const uint32_t kMagic = 0x484C4332u;   // "HLC2"
@@ -309,6 +311,7 @@ int hlc2_build_index(const double* d_ra, const double* d_dec, const int64_t* d_i
     if (!ix) return HLC2_ERR_INVALID_ARG;
     ix->magic = kMagic; ix->n = n; ix->opts = o; ix->opts.grid_like = nullptr; ix->opts.d_err_arcsec = nullptr; ix->lay = L;
     ix->d_buf = (char*)d_index_buf; ix->index_bytes = index_bytes; ix->stream = s; ix->stats_valid = false;
+    ix->d_stats = nullptr; ix->outside_box = false;
     int rc = HLC2_OK;
     auto fail = [&](int code) { delete ix; return code; };
     if (cudaGetDevice(&ix->device) != cudaSuccess) { t_last_cuda = cudaGetLastError(); return fail(HLC2_ERR_CUDA); }
@@ -317,13 +320,29 @@ int hlc2_build_index(const double* d_ra, const double* d_dec, const int64_t* d_i
     Stats* d_stats = (Stats*)(buf + L.stats);
     uint32_t nn = (uint32_t)n;
 
-    // (a1) extent pass, then plan the grid on the host (one small D2H + sync)
-    launch_stats(d_ra, d_dec, nn, d_stats, s);
-    if (cudaMemcpyAsync(&ix->h_stats, d_stats, sizeof(Stats), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
-        cudaStreamSynchronize(s) != cudaSuccess) { t_last_cuda = cudaGetLastError(); return fail(HLC2_ERR_CUDA); }
-    ix->stats_valid = true;
-    int64_t n_valid = n - (int64_t)ix->h_stats.n_bad;
-    if (o.grid_like) {
+    const bool async_like = o.grid_like && o.async_like;
+    Stats* collect = nullptr;
+    int64_t n_valid = n;
+    if (async_like) {
+        // the grid is given: no extent pass, no synchronisation.  k_keys_pack gathers the status record on the way
+        // (read by hlc2_index_status).  The declination extent only prunes windows in the two-grid planner, so the
+        // whole sphere (a superset) stands in for it; sources beyond the end zones are filed in them, as always.
+        launch_stats_init(d_stats, s);
+        collect = d_stats;
+        ix->d_stats = d_stats;
+        ix->grid = o.grid_like->grid;
+        ix->grid.dec_min = -90.0; ix->grid.dec_max = 90.0;
+    } else {
+        // (a1) extent pass, then plan the grid on the host (one small D2H + sync)
+        launch_stats(d_ra, d_dec, nn, d_stats, s);
+        if (cudaMemcpyAsync(&ix->h_stats, d_stats, sizeof(Stats), cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+            cudaStreamSynchronize(s) != cudaSuccess) { t_last_cuda = cudaGetLastError(); return fail(HLC2_ERR_CUDA); }
+        ix->stats_valid = true;
+        n_valid = n - (int64_t)ix->h_stats.n_bad;
+    }
+    if (async_like) {
+        // nothing to plan
+    } else if (o.grid_like) {
         ix->grid = o.grid_like->grid;
         if (n_valid > 0) {
             ix->grid.dec_min = f64_from_order_bits(ix->h_stats.dec_min_bits);
@@ -335,8 +354,13 @@ int hlc2_build_index(const double* d_ra, const double* d_dec, const int64_t* d_i
     }
     const HostGrid& g = ix->grid;
     if ((size_t)g.n_zones > L.cap_zones || (size_t)g.n_cells() > L.cap_cells) return fail(HLC2_ERR_BUFFER_TOO_SMALL);
-    if (cudaMemcpyAsync(buf + L.n_ra, g.n_ra.data(), (size_t)g.n_zones * 4, cudaMemcpyHostToDevice, s) != cudaSuccess ||
-        cudaMemcpyAsync(buf + L.cell_base, g.cell_base.data(), ((size_t)g.n_zones + 1) * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) {
+    // zone tables: from the host plan, or (asynchronous build) device to device from the index that owns the grid
+    const hlc2_index* like = o.grid_like;
+    const void* src_n_ra = async_like ? (const void*)(like->d_buf + like->lay.n_ra) : (const void*)g.n_ra.data();
+    const void* src_base = async_like ? (const void*)(like->d_buf + like->lay.cell_base) : (const void*)g.cell_base.data();
+    const cudaMemcpyKind kind = async_like ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    if (cudaMemcpyAsync(buf + L.n_ra, src_n_ra, (size_t)g.n_zones * 4, kind, s) != cudaSuccess ||
+        cudaMemcpyAsync(buf + L.cell_base, src_base, ((size_t)g.n_zones + 1) * 4, kind, s) != cudaSuccess) {
         t_last_cuda = cudaGetLastError(); return fail(HLC2_ERR_CUDA);
     }
     GridView gv = grid_view(ix);
@@ -355,7 +379,7 @@ int hlc2_build_index(const double* d_ra, const double* d_dec, const int64_t* d_i
     Rec* rec = (Rec*)(tmp + T.rec);
     uint32_t* digit_hist = (uint32_t*)(tmp + T.digit_hist);
     if (cudaMemsetAsync(digit_hist, 0, (size_t)kMaxPasses * kRadix * 4, s) != cudaSuccess) { t_last_cuda = cudaGetLastError(); return fail(HLC2_ERR_CUDA); }
-    launch_keys_pack(d_ra, d_dec, d_id, nn, gv, passes, o.r_max_arcsec, ix->flagged, ka, rec, digit_hist, s);
+    launch_keys_pack(d_ra, d_dec, d_id, nn, gv, passes, o.r_max_arcsec, ix->flagged, ka, rec, digit_hist, s, collect);
     int where = launch_radix_sort(ka, kb, pa, pb, nn, key_bits, digit_hist, (uint32_t*)(tmp + T.digit_base),
                                   (uint32_t*)(tmp + T.status), (uint32_t*)(tmp + T.ticket), s);
     const uint32_t* perm = where ? pb : pa;
@@ -378,6 +402,12 @@ int hlc2_index_status(const hlc2_index* idx, int64_t* first_bad_row) {
     CU(cudaStreamSynchronize(idx->stream));
     CU(cudaGetLastError());
     if (first_bad_row) *first_bad_row = -1;
+    if (idx->d_stats) {       // asynchronous build: the record lives on the device (re-read: a graph replay rewrites it)
+        hlc2_index* ix = const_cast<hlc2_index*>(idx);
+        CU(cudaMemcpy(&ix->h_stats, idx->d_stats, sizeof(Stats), cudaMemcpyDeviceToHost));
+        ix->stats_valid = true; ix->outside_box = ix->h_stats.ra_hist[0] != 0;
+    }
+    if (idx->outside_box) return HLC2_ERR_GRID_MISMATCH;
     if (idx->stats_valid && idx->h_stats.n_bad) {
         if (first_bad_row) *first_bad_row = (int64_t)idx->h_stats.first_bad_row;
         return HLC2_ERR_BAD_COORD;

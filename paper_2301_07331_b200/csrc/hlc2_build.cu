@@ -80,8 +80,10 @@ __global__ void k_stats_init(Stats* st) {
     if (i == 0) { st->dec_min_bits = ~0ull; st->dec_max_bits = 0ull; st->first_bad_row = ~0ull; st->n_bad = 0; }
 }
 
+void launch_stats_init(Stats* d_stats, cudaStream_t s) { k_stats_init<<<(kRaBins + 255) / 256, 256, 0, s>>>(d_stats); count_launch(); }
+
 void launch_stats(const double* ra, const double* dec, uint32_t n, Stats* d_stats, cudaStream_t s) {
-    k_stats_init<<<(kRaBins + 255) / 256, 256, 0, s>>>(d_stats); count_launch();
+    launch_stats_init(d_stats, s);
     if (n == 0) return;
     int blocks = (int)std::min<size_t>(((size_t)n + kStatsThreads - 1) / kStatsThreads, (size_t)sm_count() * 4);
     k_stats<<<blocks, kStatsThreads, 0, s>>>(ra, dec, n, d_stats); count_launch();
@@ -152,7 +154,10 @@ __device__ __forceinline__ uint32_t window_flags(const GridView& g, double dec, 
 __global__ void __launch_bounds__(kKeyThreads)
 k_keys_pack(const double* __restrict__ ra, const double* __restrict__ dec, const int64_t* __restrict__ id, uint32_t n,
             GridView g, int passes, double rpad_deg, double sin_r, int flagged,
-            uint32_t* __restrict__ keys, Rec* __restrict__ rec, uint32_t* __restrict__ digit_hist) {
+            uint32_t* __restrict__ keys, Rec* __restrict__ rec, uint32_t* __restrict__ digit_hist, Stats* __restrict__ st) {
+    // st != null (a build on a given grid without the extent pass): this kernel also gathers what hlc2_index_status
+    // reports -- bad rows, the declination extent, and in ra_hist[0] the sources that lie outside the grid's RA box
+    unsigned long long dmin = ~0ull, dmax = 0ull, bad_row = ~0ull; unsigned nbad = 0, nout = 0;
     __shared__ uint32_t hist[kMaxPasses * kRadix];
     for (int i = threadIdx.x; i < kMaxPasses * kRadix; i += kKeyThreads) hist[i] = 0;
     __syncthreads();
@@ -171,8 +176,14 @@ k_keys_pack(const double* __restrict__ ra, const double* __restrict__ dec, const
             const int k = cell_of_u(g, u, nra);
             key = __ldg(g.cell_base + z) + (uint32_t)k;
             unit_vector(an, d, ux, uy, uz);
+            if (st) {
+                const unsigned long long b = f64_order_bits(d);
+                dmin = min(dmin, b); dmax = max(dmax, b);
+                if (u > g.span) ++nout;
+            }
             if (flagged) flags = window_flags(g, d, sqrt(fma(ux, ux, uy * uy)), u, z, nra, k, rpad_deg, sin_r);
         }
+        else if (st) { ++nbad; bad_row = min(bad_row, (unsigned long long)i); }
         keys[i] = key | flags;          // the sort looks at the key bits only; the flags ride along
         double2* o = reinterpret_cast<double2*>(rec + i);
         o[0] = make_double2(ux, uy);
@@ -182,15 +193,26 @@ k_keys_pack(const double* __restrict__ ra, const double* __restrict__ dec, const
     __syncthreads();
     for (int i = threadIdx.x; i < passes * kRadix; i += kKeyThreads)
         if (hist[i]) atomicAdd(&digit_hist[i], hist[i]);
+    if (st) {
+        for (int o = 16; o; o >>= 1) {
+            dmin = min(dmin, __shfl_xor_sync(0xffffffffu, dmin, o)); dmax = max(dmax, __shfl_xor_sync(0xffffffffu, dmax, o));
+            nout += __shfl_xor_sync(0xffffffffu, nout, o);
+        }
+        if ((threadIdx.x & 31) == 0) {
+            if (dmin != ~0ull) { atomicMin(&st->dec_min_bits, dmin); atomicMax(&st->dec_max_bits, dmax); }
+            if (nout) atomicAdd(&st->ra_hist[0], nout);
+        }
+        if (nbad) { atomicAdd(&st->n_bad, (unsigned long long)nbad); atomicMin(&st->first_bad_row, bad_row); }
+    }
 }
 
 void launch_keys_pack(const double* ra, const double* dec, const int64_t* id, uint32_t n, GridView g, int passes,
-                      double r_max_arcsec, bool flagged, uint32_t* keys, Rec* rec, uint32_t* digit_hist, cudaStream_t s) {
+                      double r_max_arcsec, bool flagged, uint32_t* keys, Rec* rec, uint32_t* digit_hist, cudaStream_t s, Stats* collect) {
     if (n == 0) return;
     int blocks = (int)std::min<size_t>(((size_t)n + kKeyThreads - 1) / kKeyThreads, (size_t)sm_count() * 8);
     const double rpad_deg = r_max_arcsec / 3600.0 + 1e-9;
     const double sin_r = sin(r_max_arcsec * (M_PI / 648000.0)) * (1.0 + 1e-9);
-    k_keys_pack<<<blocks, kKeyThreads, 0, s>>>(ra, dec, id, n, g, passes, rpad_deg, sin_r, flagged ? 1 : 0, keys, rec, digit_hist);
+    k_keys_pack<<<blocks, kKeyThreads, 0, s>>>(ra, dec, id, n, g, passes, rpad_deg, sin_r, flagged ? 1 : 0, keys, rec, digit_hist, collect);
     count_launch();
 }
 

@@ -92,7 +92,9 @@ int current_device();
 int sm_count();
 void launch_stats(const double* ra, const double* dec, uint32_t n, Stats* d_stats, cudaStream_t s);
 void launch_keys_pack(const double* ra, const double* dec, const int64_t* id, uint32_t n, GridView g, int passes,
-                      double r_max_arcsec, bool flagged, uint32_t* keys, Rec* rec, uint32_t* digit_hist, cudaStream_t s);
+                      double r_max_arcsec, bool flagged, uint32_t* keys, Rec* rec, uint32_t* digit_hist, cudaStream_t s,
+                      Stats* collect = nullptr);
+void launch_stats_init(Stats* d_stats, cudaStream_t s);
 int  radix_passes(int key_bits);
 size_t sort_tiles(uint32_t n);
 // sorts (keys, row) by key; returns which of the double buffers holds the result (0 = a, 1 = b)
