@@ -263,6 +263,19 @@ static_assert(kOsThreads == kRadix, "one thread per digit");
 
 size_t sort_tiles(uint32_t n) { return ((size_t)n + kOsTile - 1) / kOsTile; }
 
+// lanes of the (converged) warp that hold the same value d < 2^(kRadixBits + 1), one ballot per bit.  Out of line: it is the
+// rare path of the ranking and must not cost the common one registers.
+__device__ __noinline__ unsigned match_by_votes(uint32_t d) {
+    unsigned p = 0xffffffffu;
+#pragma unroll 1
+    for (int b = 0; b <= kRadixBits; ++b) {                           // bit kRadixBits tells empty slots (all ones) apart
+        const bool bit = (d >> b) & 1u;
+        const unsigned vote = __ballot_sync(0xffffffffu, bit);
+        p &= bit ? vote : ~vote;
+    }
+    return p;
+}
+
 template <bool FirstPass>
 __global__ void __launch_bounds__(kOsThreads, 2)
 k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals, uint32_t n, int shift, uint32_t mask,
@@ -286,29 +299,56 @@ k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
     const uint32_t cnt = (uint32_t)min((size_t)kOsTile, (size_t)n - tile_base);
 
     // warp w owns kOsItems*32 consecutive keys; item r of lane l is key (w*kOsItems + r)*32 + l of the tile
-    const size_t base = tile_base + (size_t)w * (kOsItems * 32) + lane;
-    uint32_t k[kOsItems], v[kOsItems], rk[kOsItems / 2];      // ranks (< kOsTile) packed two per register
+    const uint32_t t0 = (uint32_t)w * (kOsItems * 32) + lane;         // slot of item r in the tile: t0 + 32 r
+    const uint32_t* tkeys = keys + tile_base;
+    // the rows (vals) are not held across the ranking: they are read when the reorder needs them, which keeps the
+    // kernel inside 64 registers without spills
+    uint32_t k[kOsItems], rk[kOsItems / 2];                   // ranks (< kOsTile) packed two per register
 #pragma unroll
     for (int r = 0; r < kOsItems; ++r) {
-        size_t i = base + (size_t)r * 32;
-        k[r] = i < n ? __ldg(keys + i) : 0xFFFFFFFFu;
-        v[r] = FirstPass ? (uint32_t)i : (i < n ? __ldg(vals + i) : 0u);
+        const uint32_t t = t0 + r * 32;
+        k[r] = t < cnt ? __ldg(tkeys + t) : 0xFFFFFFFFu;
     }
     const unsigned lt = (1u << lane) - 1;
     uint32_t* mywh = wh + w * kRadix;
-    // ranks, six items at a time in three phases (all matches, then all counter bumps, then all broadcasts), so that the
-    // latencies of match_any, of the shared-memory atomics and of the shuffles overlap instead of adding up item by item
-    constexpr int kG = 6;
+    // ranks, kG items at a time in phases (tags, matches, counter bumps, broadcasts), so that the latencies of the
+    // shared-memory accesses, of the atomics and of the shuffles overlap instead of adding up item by item.
+    // No MATCH.ANY: it measures 48 cycles per warp instruction per SM on sm_100a and alone was half of this kernel's time
+    // (profiles/r2_build_experiments.md); nine ballots (one per digit bit) measure 20, the owner tags below about half of that.
+#ifndef HLC2_OS_GROUP
+#define HLC2_OS_GROUP 2
+#endif
+    constexpr int kG = HLC2_OS_GROUP;
     static_assert(kOsItems % kG == 0, "items are ranked in groups");
 #pragma unroll
     for (int g = 0; g < kOsItems; g += kG) {
         uint32_t d[kG]; unsigned peers[kG]; uint32_t old[kG];
+        // owner tags: every lane writes its number under its digit in a table of the warp's own and reads it back; a lane
+        // that reads another lane's number shares its digit with it.  Only those digits (one per item on average with 32
+        // keys over 512 digits) are then settled by a vote each; everybody else is alone and needs no vote at all.
+        uint8_t* own = reinterpret_cast<uint8_t*>(s_keys) + (size_t)(w * kG) * kRadix;     // the staging area is free until the reorder
 #pragma unroll
         for (int j = 0; j < kG; ++j) {
-            const bool ok = base + (size_t)(g + j) * 32 < n;
+            const bool ok = t0 + (g + j) * 32 < cnt;
             d[j] = ok ? ((k[g + j] >> shift) & mask) : 0xFFFFFFFFu;
-            peers[j] = __match_any_sync(0xffffffffu, d[j]);
+            if (ok) own[j * kRadix + d[j]] = (uint8_t)lane;
         }
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < kG; ++j) {
+            const bool lost = d[j] != 0xFFFFFFFFu && own[j * kRadix + d[j]] != (uint8_t)lane;
+            unsigned open = __ballot_sync(0xffffffffu, lost);
+            peers[j] = 1u << lane;
+            // many shared digits (a dense cell, sorted input): one vote per digit bit settles them all at once
+            if (__popc(open) > 8) { peers[j] = match_by_votes(d[j]); open = 0; }
+            while (open) {
+                const uint32_t dl = __shfl_sync(0xffffffffu, d[j], __ffs(open) - 1);
+                const unsigned grp = __ballot_sync(0xffffffffu, d[j] == dl);
+                if (d[j] == dl) peers[j] = grp;
+                open &= ~grp;
+            }
+        }
+        __syncwarp();                                                 // the next group reuses the tables
         // lanes with the same digit: the lowest of them bumps the warp's counter once for all and hands the old value
         // round; the groups of one step are disjoint digits or the same counter in program order: atomics keep it exact
 #pragma unroll
@@ -334,6 +374,32 @@ k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
     *my_status = c | (tile == 0 ? kFlagIncl : kFlagAgg);
     uint32_t tot;
     const uint32_t loc = block_scan_incl(c, &tot, s_scan) - c;      // first position of digit d in the sorted tile
+#pragma unroll
+    for (int ww = 0; ww < kOsWarps; ++ww) wh[ww * kRadix + dgt] += loc;
+    __syncthreads();
+
+    // the reorder in shared memory needs tile-local offsets only: it runs BEFORE the look-back, so that the tiles ahead
+    // (which started earlier) have had that much longer to publish their inclusive prefixes and the walk stays short
+    constexpr int kV = 6;
+#pragma unroll
+    for (int g = 0; g < kOsItems; g += kV) {
+        uint32_t v[kV];
+#pragma unroll
+        for (int j = 0; j < kV; ++j) {
+            const uint32_t t = t0 + (g + j) * 32;
+            v[j] = FirstPass ? (uint32_t)tile_base + t : (t < cnt ? __ldg(vals + tile_base + t) : 0u);
+        }
+#pragma unroll
+        for (int j = 0; j < kV; ++j) {
+            const int r = g + j;
+            if (t0 + r * 32 < cnt) {
+                const uint32_t d = (k[r] >> shift) & mask;
+                const uint32_t pos = mywh[d] + ((rk[r >> 1] >> (16 * (r & 1))) & 0xFFFFu);
+                s_keys[pos] = k[r]; s_vals[pos] = v[j];
+            }
+        }
+    }
+
     uint32_t excl = 0;
     if (tile > 0) {
         // look back over the predecessors' records, eight at a time (independent loads: one memory latency per eight
@@ -356,18 +422,6 @@ k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
         *my_status = (excl + c) | kFlagIncl;
     }
     s_gbase[dgt] = __ldg(digit_base + dgt) + excl - loc;            // global slot of sorted-tile position j is s_gbase[d] + j
-#pragma unroll
-    for (int ww = 0; ww < kOsWarps; ++ww) wh[ww * kRadix + dgt] += loc;
-    __syncthreads();
-
-#pragma unroll
-    for (int r = 0; r < kOsItems; ++r) {
-        if (base + (size_t)r * 32 < n) {
-            const uint32_t d = (k[r] >> shift) & mask;
-            const uint32_t pos = mywh[d] + ((rk[r >> 1] >> (16 * (r & 1))) & 0xFFFFu);
-            s_keys[pos] = k[r]; s_vals[pos] = v[r];
-        }
-    }
     __syncthreads();
     for (uint32_t j = threadIdx.x; j < cnt; j += kOsThreads) {
         const uint32_t key = s_keys[j];
