@@ -60,7 +60,8 @@ typedef enum {
     HLC2_ERR_BAD_COORD = -4,         /* a non-finite coordinate or |dec| > 90 was found (hlc2_index_status) */
     HLC2_ERR_CUDA = -5,              /* a CUDA runtime call failed; see hlc2_last_cuda_error */
     HLC2_ERR_GRID_MISMATCH = -6,     /* opts.grid_like: the catalogue does not fit inside that grid's box */
-    HLC2_ERR_TOO_MANY = -7           /* n >= 2^30 sources in one index (stream the catalogue instead) */
+    HLC2_ERR_TOO_MANY = -7,          /* n >= 2^30 sources in one index (stream the catalogue instead) */
+    HLC2_ERR_STATIC_LIMIT = -8       /* hlc2_crossmatch_static: the match needs more than HLC2_STATIC_SCRATCH_BYTES */
 } hlc2_status;
 
 /*
@@ -198,6 +199,25 @@ int hlc2_crossmatch_events(const hlc2_index* A, const hlc2_index* B, double radi
                            int64_t capacity, unsigned long long* d_count,
                            void* d_temp, size_t temp_bytes, void* cuda_stream,
                            void* ev_kernel_start, void* ev_kernel_stop);
+
+/*
+ * hlc2_crossmatch for callers that can neither allocate device memory nor carry a scratch buffer (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): same operation, same results, same arguments minus
+ * d_temp / temp_bytes.  The scratch (the planner's job lists, the general-row list: SURVEY 8(a5)-(a7)) lives in a static
+ * device array of HLC2_STATIC_SCRATCH_BYTES inside the library, which every GPU that loads the library holds until the
+ * process exits.  The call makes no cudaMalloc / cudaFree and calls no allocating library routine.
+ *   Limit: hlc2_crossmatch_sizes(A, B) <= HLC2_STATIC_SCRATCH_BYTES, i.e. A of up to about 2 million rows (4 bytes per
+ *   A row + 256, or the planner's lists if larger); beyond it the call returns HLC2_ERR_STATIC_LIMIT and does nothing.
+ *   Sharing: all calls on one device use the same array.  Calls that may OVERLAP on the GPU (different streams without an
+ *   ordering between them) race on it and give undefined results: order them, or use hlc2_crossmatch with buffers of
+ *   their own.  The array keeps the previous call's contents; each call clears the counters it keeps there itself.
+ *   The first call on a device resolves the array's device address (cudaGetSymbolAddress, the device of the indices
+ *   current): make one call before starting a stream capture.  Other errors and stream behaviour as hlc2_crossmatch.
+ */
+#define HLC2_STATIC_SCRATCH_BYTES (8u << 20)
+int hlc2_crossmatch_static(const hlc2_index* A, const hlc2_index* B, double radius_arcsec, int mode,
+                           int64_t* d_out_idA, int64_t* d_out_idB, double* d_out_sep_arcsec,
+                           int64_t capacity, unsigned long long* d_count, void* cuda_stream);
 
 /*
  * Self-match of ONE catalogue (the paper's D4 case: 2MASS against itself, Table 2).

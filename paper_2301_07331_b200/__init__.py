@@ -27,6 +27,8 @@ HLC2_ERR_BAD_COORD = -4
 HLC2_ERR_CUDA = -5
 HLC2_ERR_GRID_MISMATCH = -6
 HLC2_ERR_TOO_MANY = -7
+HLC2_ERR_STATIC_LIMIT = -8
+HLC2_STATIC_SCRATCH_BYTES = 8 << 20
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libhlc2.so")
@@ -86,6 +88,7 @@ def lib():
         L.hlc2_crossmatch_events.argtypes = L.hlc2_crossmatch.argtypes + [vp, vp]
         L.hlc2_selfmatch.argtypes = [vp, ctypes.c_double, ctypes.c_int, ctypes.c_int, vp, vp, vp, i64, vp, vp, sz, vp]
         L.hlc2_crossmatch_radii.argtypes = [vp, vp, ctypes.c_double, ctypes.c_double, ctypes.c_int, vp, vp, vp, i64, vp, vp, sz, vp]
+        L.hlc2_crossmatch_static.argtypes = [vp, vp, ctypes.c_double, ctypes.c_int, vp, vp, vp, i64, vp, vp]
         L.hlc2_version.restype = ctypes.c_char_p
         _lib = L
     return _lib
@@ -248,6 +251,17 @@ def hlc2_crossmatch(A: Index, B: Index, radius_arcsec: float, mode: int, out_ida
         rc = lib().hlc2_crossmatch_events(*args, e0, e1)
     if rc != HLC2_OK:
         raise Hlc2Error(rc, "hlc2_crossmatch")
+
+
+def hlc2_crossmatch_static(A: Index, B: Index, radius_arcsec: float, mode: int, out_ida, out_idb, out_sep, count, stream=None):
+    """hlc2_crossmatch with the library's static scratch array (no device allocation anywhere in the call; this wrapper
+    makes none either).  Raises Hlc2Error(HLC2_ERR_STATIC_LIMIT) when the match needs more than HLC2_STATIC_SCRATCH_BYTES."""
+    cap = int(out_ida.shape[0])
+    assert out_idb.shape[0] == cap and out_sep.shape[0] == cap
+    rc = lib().hlc2_crossmatch_static(A.handle, B.handle, float(radius_arcsec), int(mode), out_ida.data_ptr(), out_idb.data_ptr(),
+                                      out_sep.data_ptr(), cap, count.data_ptr(), _stream_ptr(stream))
+    if rc != HLC2_OK:
+        raise Hlc2Error(rc, "hlc2_crossmatch_static")
 
 
 def _run_sized(call, n_hint: int, dev, capacity):

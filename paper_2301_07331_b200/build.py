@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 SO = os.path.join(HERE, "libhlc2.so")
-SOURCES = ["hlc2_api.cu", "hlc2_build.cu", "hlc2_match.cu", "hlc2_match_same.cu", "hlc2_stream.cu"]
+SOURCES = ["hlc2_api.cu", "hlc2_build.cu", "hlc2_match.cu", "hlc2_match_same.cu", "hlc2_stream.cu", "hlc2_static.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
 

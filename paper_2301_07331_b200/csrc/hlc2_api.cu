@@ -17,6 +17,7 @@ namespace hlc2 {
 static std::atomic<unsigned long long> g_launches{0};
 void count_launch(int k) { g_launches.fetch_add((unsigned long long)k, std::memory_order_relaxed); }
 static thread_local cudaError_t t_last_cuda = cudaSuccess;
+void note_cuda_error(cudaError_t e) { t_last_cuda = e; }      // for the entry points that live in other files
 }  // namespace hlc2
 
 #define CU(call)                                                    \
@@ -526,6 +527,7 @@ const char* hlc2_strerror(int status) {
         case HLC2_ERR_CUDA: return "CUDA runtime error (see hlc2_last_cuda_error)";
         case HLC2_ERR_GRID_MISMATCH: return "catalogue does not fit inside the grid_like index's RA box";
         case HLC2_ERR_TOO_MANY: return "too many sources for one index (>= 2^30)";
+        case HLC2_ERR_STATIC_LIMIT: return "hlc2_crossmatch_static: the match needs more scratch than the static array holds (HLC2_STATIC_SCRATCH_BYTES = 8 MiB, about 2 million A rows); use hlc2_crossmatch with a caller buffer";
         default: return "unknown status";
     }
 }

@@ -95,6 +95,7 @@ void launch_keys_pack(const double* ra, const double* dec, const int64_t* id, ui
                       double r_max_arcsec, bool flagged, uint32_t* keys, Rec* rec, uint32_t* digit_hist, cudaStream_t s,
                       Stats* collect = nullptr);
 void launch_stats_init(Stats* d_stats, cudaStream_t s);
+void note_cuda_error(cudaError_t e);          // what hlc2_last_cuda_error reports (thread-local, hlc2_api.cu)
 int  radix_passes(int key_bits);
 size_t sort_tiles(uint32_t n);
 // sorts (keys, row) by key; returns which of the double buffers holds the result (0 = a, 1 = b)
