@@ -209,7 +209,10 @@ k_keys_pack(const double* __restrict__ ra, const double* __restrict__ dec, const
 void launch_keys_pack(const double* ra, const double* dec, const int64_t* id, uint32_t n, GridView g, int passes,
                       double r_max_arcsec, bool flagged, uint32_t* keys, Rec* rec, uint32_t* digit_hist, cudaStream_t s, Stats* collect) {
     if (n == 0) return;
-    int blocks = (int)std::min<size_t>(((size_t)n + kKeyThreads - 1) / kKeyThreads, (size_t)sm_count() * 8);
+#ifndef HLC2_KEYS_CTAS
+#define HLC2_KEYS_CTAS 32
+#endif
+    int blocks = (int)std::min<size_t>(((size_t)n + kKeyThreads - 1) / kKeyThreads, (size_t)sm_count() * HLC2_KEYS_CTAS);
     const double rpad_deg = r_max_arcsec / 3600.0 + 1e-9;
     const double sin_r = sin(r_max_arcsec * (M_PI / 648000.0)) * (1.0 + 1e-9);
     k_keys_pack<<<blocks, kKeyThreads, 0, s>>>(ra, dec, id, n, g, passes, rpad_deg, sin_r, flagged ? 1 : 0, keys, rec, digit_hist, collect);
@@ -468,6 +471,21 @@ int launch_radix_sort(uint32_t* keys_a, uint32_t* keys_b, uint32_t* val_a, uint3
 // ------------------------------------------------------------------------------------------
 // (a3) gather: sorted row order -> SoA unit vectors + ids.  One 32-byte sector per source.
 // ------------------------------------------------------------------------------------------
+__device__ __forceinline__ float2 pos_estimate(double x, double y, double z) {
+    // fp32 (ra, dec) estimate of the sorted row: the two-grid match locates its search window from it (padded by the
+    // error bound of exactly this chain); this kernel waits on scattered lines, so the two atan2f
+    // are free here and are paid once per build, not per match
+    const float fx = (float)x, fy = (float)y, fz = (float)z;
+    const float rxy = sqrtf(fx * fx + fy * fy);
+    float ra_f = atan2f(fy, fx) * 57.29577951f;
+    if (ra_f < 0.0f) ra_f += 360.0f;
+    return make_float2(ra_f, atan2f(fz, rxy) * 57.29577951f);
+}
+
+// A random 32-byte record costs a whole 128-byte line of DRAM traffic on this part whatever its neighbours do
+// (profiles/r2_build_experiments.md): the kernel is bound by line fetches in flight.  One row per thread and a grid far
+// larger than what is resident measured best (2.9 ms per 1e8 rows; 16 persistent CTAs per SM: 3.5 ms, their last
+// wave leaves a third of the SM idle; two or four rows per thread: 3.0-3.8 ms).
 __global__ void __launch_bounds__(256)
 k_gather(const Rec* __restrict__ rec, const uint32_t* __restrict__ perm, uint32_t n,
          double* __restrict__ x, double* __restrict__ y, double* __restrict__ z, int64_t* __restrict__ out_id,
@@ -476,21 +494,14 @@ k_gather(const Rec* __restrict__ rec, const uint32_t* __restrict__ perm, uint32_
         const double2* q = reinterpret_cast<const double2*>(rec + __ldg(perm + i));
         const double2 a = __ldg(q), b = __ldg(q + 1);
         x[i] = a.x; y[i] = a.y; z[i] = b.x; out_id[i] = __double_as_longlong(b.y);
-        // fp32 (ra, dec) estimate of the sorted row: the match kernel locates its search window from it
-        // (padded by the error bound of exactly this chain); this kernel waits on
-        // scattered sectors, so the two atan2f are free here and are paid once per build, not per match
-        const float fx = (float)a.x, fy = (float)a.y, fz = (float)b.x;
-        const float rxy = sqrtf(fx * fx + fy * fy);
-        float ra_f = atan2f(fy, fx) * 57.29577951f;
-        if (ra_f < 0.0f) ra_f += 360.0f;
-        pos[i] = make_float2(ra_f, atan2f(fz, rxy) * 57.29577951f);
+        pos[i] = pos_estimate(a.x, a.y, b.x);
     }
 }
 
 void launch_gather(const Rec* rec, const uint32_t* perm, uint32_t n, double* x, double* y, double* z, int64_t* out_id,
                    float2* pos, cudaStream_t s) {
     if (n == 0) return;
-    int blocks = (int)std::min<size_t>(((size_t)n + 255) / 256, (size_t)sm_count() * 16);
+    int blocks = (int)std::min<size_t>(((size_t)n + 255) / 256, (size_t)sm_count() * 4096);
     k_gather<<<blocks, 256, 0, s>>>(rec, perm, n, x, y, z, out_id, pos); count_launch();
 }
 
