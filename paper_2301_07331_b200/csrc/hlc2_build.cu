@@ -98,28 +98,31 @@ void launch_stats(const double* ra, const double* dec, uint32_t n, Stats* d_stat
 // sin and cos of |x| <= pi/4 without range reduction: the classic minimax polynomials of that interval (Cephes
 // sin.c / cos.c coefficients; |error| < 1.2e-16, sin keeps full relative accuracy for tiny x).  The arguments here are
 // already reduced in the degree domain, so the library sincos' reduction and special cases are dead weight.
+// The fp64 literals of this kernel live in constant memory on purpose: as immediates every one of them costs two 32-bit
+// moves per use (74 of the key pass's 330 instructions per source were such moves), as c[bank][offset] operands none.
+__constant__ double kSinPoly[6] = {1.58962301576546568060e-10, -2.50507477628578072866e-8, 2.75573136213857245213e-6,
+                                   -1.98412698295895385996e-4, 8.33333333332211858878e-3, -1.66666666666666307295e-1};
+__constant__ double kCosPoly[6] = {-1.13585365213876817300e-11, 2.08757008419747316778e-9, -2.75573141792967388112e-7,
+                                   2.48015872888517045348e-5, -1.38888888888730564116e-3, 4.16666666666665929218e-2};
+__constant__ double kTrig[4] = {0.017453292519943295 /* pi / 180 */, 1.0 / 90.0, -90.0, 57.29577951308232};
+
 __device__ __forceinline__ void sincos_quarter(double x, double& s, double& c) {
     const double z = x * x;
-    double ps = 1.58962301576546568060e-10;
-    ps = fma(ps, z, -2.50507477628578072866e-8);
-    ps = fma(ps, z, 2.75573136213857245213e-6);
-    ps = fma(ps, z, -1.98412698295895385996e-4);
-    ps = fma(ps, z, 8.33333333332211858878e-3);
-    ps = fma(ps, z, -1.66666666666666307295e-1);
+    double ps = kSinPoly[0];
+#pragma unroll
+    for (int i = 1; i < 6; ++i) ps = fma(ps, z, kSinPoly[i]);
     s = fma(x * z, ps, x);
-    double pc = -1.13585365213876817300e-11;
-    pc = fma(pc, z, 2.08757008419747316778e-9);
-    pc = fma(pc, z, -2.75573141792967388112e-7);
-    pc = fma(pc, z, 2.48015872888517045348e-5);
-    pc = fma(pc, z, -1.38888888888730564116e-3);
-    pc = fma(pc, z, 4.16666666666665929218e-2);
+    double pc = kCosPoly[0];
+#pragma unroll
+    for (int i = 1; i < 6; ++i) pc = fma(pc, z, kCosPoly[i]);
     c = fma(z * z, pc, fma(-0.5, z, 1.0));
 }
 
-__device__ __forceinline__ void unit_vector(double ra_norm, double dec, double& x, double& y, double& z) {
-    const double D2R = 0.017453292519943295;   // pi / 180
-    double q = rint(ra_norm * (1.0 / 90.0));
-    double t = fma(-90.0, q, ra_norm);
+// also returns cos(dec) (>= 0), which the window flags need
+__device__ __forceinline__ double unit_vector(double ra_norm, double dec, double& x, double& y, double& z) {
+    const double D2R = kTrig[0];
+    double q = rint(ra_norm * kTrig[1]);
+    double t = fma(kTrig[2], q, ra_norm);
     double st, ct; sincos_quarter(t * D2R, st, ct);
     int iq = ((int)q) & 3;
     double ca = (iq == 0) ? ct : (iq == 1) ? -st : (iq == 2) ? -ct : st;
@@ -129,6 +132,7 @@ __device__ __forceinline__ void unit_vector(double ra_norm, double dec, double& 
     double s, c; sincos_quarter((polar ? 90.0 - ad : ad) * D2R, s, c);
     const double sd = copysign(polar ? c : s, dec), cd = polar ? s : c;
     x = cd * ca; y = cd * sa; z = sd;
+    return cd;
 }
 
 constexpr int kKeyThreads = 256;
@@ -141,9 +145,12 @@ __device__ __forceinline__ uint32_t window_flags(const GridView& g, double dec, 
                                                  double rpad_deg, double sin_r) {
     const int zl = zone_of(g, dec - rpad_deg), zh = zone_of(g, dec + rpad_deg);
     if (zl < z - 1 || zh > z + 1) return kKeyGeneral;
-    const double s = sin_r / fmax(cd, 1e-300);                       // sin of the RA half-window
-    if (!(s < 0.2)) return kKeyGeneral;                               // polar rows: wide windows, rings
-    const double w = fma(0.2 * s * s, s, s) * 57.29577951308232 + 1e-9;   // asin(s) <= s + s^3 / 5 below 0.2
+    // sin of the RA half-window, in fp32 rounded up (conversions and the approximate division stay below 1e-6 relative;
+    // flags only have to be a superset): an fp64 division costs as much as one of this kernel's sincos
+    const float sf = __fdividef((float)sin_r, (float)cd) * 1.000002f;    // cd = 0 (a pole): inf, the general path
+    if (!(sf < 0.2f)) return kKeyGeneral;                             // polar rows: wide windows, rings
+    const double s = (double)sf;
+    const double w = fma(0.2 * s * s, s, s) * kTrig[3] + 1e-9;         // asin(s) <= s + s^3 / 5 below 0.2
     const double ulo = u - w, uhi = u + w;
     if (ulo < 0.0 ? ulo + 360.0 <= g.span : uhi >= 360.0) return kKeyGeneral;  // the window's image through RA = 0/360 lies inside the box
     const int klo = cell_of_u(g, fmax(ulo, 0.0), nra), khi = cell_of_u(g, fmin(uhi, g.span), nra);
@@ -161,9 +168,16 @@ k_keys_pack(const double* __restrict__ ra, const double* __restrict__ dec, const
     __shared__ uint32_t hist[kMaxPasses * kRadix];
     for (int i = threadIdx.x; i < kMaxPasses * kRadix; i += kKeyThreads) hist[i] = 0;
     __syncthreads();
-    for (size_t i = (size_t)blockIdx.x * kKeyThreads + threadIdx.x; i < n; i += (size_t)gridDim.x * kKeyThreads) {
-        double a = __ldg(ra + i), d = __ldg(dec + i);
-        long long v = id ? (long long)__ldg(id + i) : (long long)i;
+    // the loads of the next source are issued before the ~300 instructions of this one: without that a warp has nothing
+    // in flight while it computes, and the pass waits on memory latency at half occupancy
+    const size_t step = (size_t)gridDim.x * kKeyThreads;
+    size_t i = (size_t)blockIdx.x * kKeyThreads + threadIdx.x;
+    double a_next = 0.0, d_next = 0.0; long long v_next = 0;
+    if (i < n) { a_next = __ldg(ra + i); d_next = __ldg(dec + i); v_next = id ? (long long)__ldg(id + i) : (long long)i; }
+    for (; i < n; i += step) {
+        const double a = a_next, d = d_next;
+        const long long v = v_next;
+        if (i + step < n) { a_next = __ldg(ra + i + step); d_next = __ldg(dec + i + step); v_next = id ? (long long)__ldg(id + i + step) : (long long)(i + step); }
         uint32_t key = 0, flags = 0;
         // bad coordinate: NaN components, so that no chord test against anything (another bad row, the match's
         // sentinel slot) can pass; such rows are filed under cell 0 and never appear in a result
@@ -175,13 +189,13 @@ k_keys_pack(const double* __restrict__ ra, const double* __restrict__ dec, const
             const double u = box_u(g, an);
             const int k = cell_of_u(g, u, nra);
             key = __ldg(g.cell_base + z) + (uint32_t)k;
-            unit_vector(an, d, ux, uy, uz);
+            const double cd = unit_vector(an, d, ux, uy, uz);
             if (st) {
                 const unsigned long long b = f64_order_bits(d);
                 dmin = min(dmin, b); dmax = max(dmax, b);
                 if (u > g.span) ++nout;
             }
-            if (flagged) flags = window_flags(g, d, sqrt(fma(ux, ux, uy * uy)), u, z, nra, k, rpad_deg, sin_r);
+            if (flagged) flags = window_flags(g, d, cd, u, z, nra, k, rpad_deg, sin_r);
         }
         else if (st) { ++nbad; bad_row = min(bad_row, (unsigned long long)i); }
         keys[i] = key | flags;          // the sort looks at the key bits only; the flags ride along
@@ -618,7 +632,10 @@ void launch_cell_table(const uint32_t* sorted_keys, uint32_t key_mask, uint32_t 
     const uint32_t cap = (uint32_t)cell_big_cap(n_cells);
     uint32_t* d_count = d_big + 3 * (size_t)cap;
     cudaMemsetAsync(d_count, 0, sizeof(uint32_t), s);
-    int blocks = (int)std::min<size_t>(((size_t)n + 1 + 1023) / 1024, (size_t)sm_count() * 16);
+#ifndef HLC2_FILL_CTAS
+#define HLC2_FILL_CTAS 64
+#endif
+    int blocks = (int)std::min<size_t>(((size_t)n + 1 + 1023) / 1024, (size_t)sm_count() * HLC2_FILL_CTAS);
     k_cell_fill<<<blocks, 256, 0, s>>>(sorted_keys, key_mask, n, n_cells, cell_start, d_big, d_count, cap); count_launch();
     k_cell_fill_big<<<sm_count() * 4, 256, 0, s>>>(d_big, d_count, cap, cell_start); count_launch();
 }
@@ -683,7 +700,10 @@ k_tile_desc(const uint32_t* __restrict__ tile_first, uint32_t n_zones, const uin
 void launch_tiles(const uint32_t* cell_start, const uint32_t* cell_base, const int32_t* n_ra, uint32_t n_zones, const uint32_t* sorted_keys,
                   uint32_t key_mask, uint32_t tile_cap, uint32_t* d_tile_first, TileDesc* tiles, uint32_t* d_n_tiles, cudaStream_t s) {
     k_zone_tiles<<<1, 1024, 0, s>>>(cell_start, cell_base, n_zones, d_tile_first, d_n_tiles); count_launch();
-    int blocks = (int)std::min<size_t>(((size_t)tile_cap + 7) / 8, (size_t)sm_count() * 8);
+#ifndef HLC2_TILE_CTAS
+#define HLC2_TILE_CTAS 64
+#endif
+    int blocks = (int)std::min<size_t>(((size_t)tile_cap + 7) / 8, (size_t)sm_count() * HLC2_TILE_CTAS);
     k_tile_desc<<<std::max(blocks, 1), 256, 0, s>>>(d_tile_first, n_zones, cell_start, cell_base, reinterpret_cast<const uint32_t*>(n_ra), sorted_keys, key_mask, tiles); count_launch();
 }
 
