@@ -267,7 +267,12 @@ k_digit_scan(const uint32_t* __restrict__ digit_hist, uint32_t* __restrict__ dig
     }
 }
 
-constexpr int kOsThreads = 512;                 // == kRadix: thread d owns digit d in the tile-level scans
+#ifndef HLC2_OS_THREADS
+#define HLC2_OS_THREADS 512
+#endif
+constexpr int kOsThreads = HLC2_OS_THREADS;     // thread t owns digits t * kOsDig .. in the tile-level scans
+constexpr int kOsDig = kRadix / kOsThreads;
+constexpr int kOsCtas = 1024 / kOsThreads;      // CTAs per SM the kernel is sized for
 #ifndef HLC2_OS_ITEMS
 #define HLC2_OS_ITEMS 18
 #endif
@@ -276,7 +281,7 @@ constexpr int kOsTile = kOsThreads * kOsItems;  // 9216 keys per tile
 constexpr int kOsWarps = kOsThreads / 32;
 constexpr uint32_t kFlagAgg = 1u << 30, kFlagIncl = 2u << 30, kFlagMask = 3u << 30;
 constexpr size_t kOsSmem = (size_t)(kOsWarps * kRadix + 2 * kOsTile) * 4;
-static_assert(kOsThreads == kRadix, "one thread per digit");
+static_assert(kOsThreads * kOsDig == kRadix && kOsDig >= 1, "whole digits per thread");
 
 size_t sort_tiles(uint32_t n) { return ((size_t)n + kOsTile - 1) / kOsTile; }
 
@@ -294,7 +299,7 @@ __device__ __noinline__ unsigned match_by_votes(uint32_t d) {
 }
 
 template <bool FirstPass>
-__global__ void __launch_bounds__(kOsThreads, 2)
+__global__ void __launch_bounds__(kOsThreads, kOsCtas)
 k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals, uint32_t n, int shift, uint32_t mask,
            const uint32_t* __restrict__ digit_base, volatile uint32_t* __restrict__ status, uint32_t* __restrict__ ticket,
            uint32_t* __restrict__ out_keys, uint32_t* __restrict__ out_vals) {
@@ -382,17 +387,26 @@ k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
     }
     __syncthreads();
 
-    // digit d = threadIdx.x: exclusive scan over the warps, tile count, chained scan over the tiles
-    const int dgt = threadIdx.x;
-    uint32_t c = 0;
+    // digits threadIdx.x * kOsDig ..: exclusive scan over the warps, tile count, chained scan over the tiles
+    const int dgt0 = threadIdx.x * kOsDig;
+    uint32_t c[kOsDig], loc[kOsDig], csum = 0;
 #pragma unroll
-    for (int ww = 0; ww < kOsWarps; ++ww) { uint32_t t = wh[ww * kRadix + dgt]; wh[ww * kRadix + dgt] = c; c += t; }
-    volatile uint32_t* my_status = status + (size_t)tile * kRadix + dgt;
-    *my_status = c | (tile == 0 ? kFlagIncl : kFlagAgg);
+    for (int q = 0; q < kOsDig; ++q) {
+        const int dgt = dgt0 + q;
+        uint32_t cc = 0;
+#pragma unroll
+        for (int ww = 0; ww < kOsWarps; ++ww) { uint32_t t = wh[ww * kRadix + dgt]; wh[ww * kRadix + dgt] = cc; cc += t; }
+        c[q] = cc; csum += cc;
+        status[(size_t)tile * kRadix + dgt] = cc | (tile == 0 ? kFlagIncl : kFlagAgg);
+    }
     uint32_t tot;
-    const uint32_t loc = block_scan_incl(c, &tot, s_scan) - c;      // first position of digit d in the sorted tile
+    uint32_t run = block_scan_incl(csum, &tot, s_scan) - csum;      // first position of the thread's first digit in the sorted tile
 #pragma unroll
-    for (int ww = 0; ww < kOsWarps; ++ww) wh[ww * kRadix + dgt] += loc;
+    for (int q = 0; q < kOsDig; ++q) {
+        loc[q] = run; run += c[q];
+#pragma unroll
+        for (int ww = 0; ww < kOsWarps; ++ww) wh[ww * kRadix + dgt0 + q] += loc[q];
+    }
     __syncthreads();
 
     // the reorder in shared memory needs tile-local offsets only: it runs BEFORE the look-back, so that the tiles ahead
@@ -417,28 +431,46 @@ k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
         }
     }
 
-    uint32_t excl = 0;
+    uint32_t excl[kOsDig];
+#pragma unroll
+    for (int q = 0; q < kOsDig; ++q) excl[q] = 0;
     if (tile > 0) {
         // look back over the predecessors' records, eight at a time (independent loads: one memory latency per eight
         // tiles instead of one per tile); stop at the first inclusive prefix, re-poll from the first record not yet there
-        long long q = (long long)tile - 1;
-        for (bool done = false; !done;) {
-            uint32_t sv[8];
+        long long at[kOsDig]; bool done[kOsDig]; bool all = false;
 #pragma unroll
-            for (int j = 0; j < 8; ++j) { sv[j] = 2u << 30; if (q - j >= 0) sv[j] = status[(size_t)(q - j) * kRadix + dgt]; }     // before tile 0: an empty inclusive prefix
-            int used = 8;
+        for (int q = 0; q < kOsDig; ++q) { at[q] = (long long)tile - 1; done[q] = false; }
+        while (!all) {
+            uint32_t sv[kOsDig][8];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                if (done || used != 8) continue;
-                if ((sv[j] & kFlagMask) == 0) { used = j; continue; }
-                excl += sv[j] & ~kFlagMask;
-                if (sv[j] & kFlagIncl) done = true;
+            for (int q = 0; q < kOsDig; ++q)
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    sv[q][j] = 2u << 30;                             // before tile 0: an empty inclusive prefix
+                    if (!done[q] && at[q] - j >= 0) sv[q][j] = status[(size_t)(at[q] - j) * kRadix + dgt0 + q];
+                }
+            all = true;
+#pragma unroll
+            for (int q = 0; q < kOsDig; ++q) {
+                if (done[q]) continue;
+                int used = 8;
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    if (done[q] || used != 8) continue;
+                    if ((sv[q][j] & kFlagMask) == 0) { used = j; continue; }
+                    excl[q] += sv[q][j] & ~kFlagMask;
+                    if (sv[q][j] & kFlagIncl) done[q] = true;
+                }
+                at[q] -= used;
+                all = all && done[q];
             }
-            q -= used;
         }
-        *my_status = (excl + c) | kFlagIncl;
+#pragma unroll
+        for (int q = 0; q < kOsDig; ++q) status[(size_t)tile * kRadix + dgt0 + q] = (excl[q] + c[q]) | kFlagIncl;
     }
-    s_gbase[dgt] = __ldg(digit_base + dgt) + excl - loc;            // global slot of sorted-tile position j is s_gbase[d] + j
+#pragma unroll
+    for (int q = 0; q < kOsDig; ++q)                                 // global slot of sorted-tile position j is s_gbase[d] + j
+        s_gbase[dgt0 + q] = __ldg(digit_base + dgt0 + q) + excl[q] - loc[q];
     __syncthreads();
     for (uint32_t j = threadIdx.x; j < cnt; j += kOsThreads) {
         const uint32_t key = s_keys[j];
