@@ -97,7 +97,11 @@ typedef struct {
                                         (everything is enqueued on the stream; the call can be captured in a CUDA graph).
                                         Bad coordinates and a catalogue that does not fit the grid's RA box are then both
                                         reported by hlc2_index_status (HLC2_ERR_BAD_COORD / HLC2_ERR_GRID_MISMATCH), not by
-                                        the build call; sources outside the box are filed in the box's last cell. */
+                                        the build call; sources outside the box are filed in the box's last cell.
+                                        The index's declination extent is taken as the whole sphere: matched against an
+                                        index on ANOTHER grid, the tiles of its first and last zone then plan windows over
+                                        every zone of that index beyond the grid (same results, more work); on the same
+                                        grid nothing changes. */
     int32_t reserved;
 } hlc2_opts;
 

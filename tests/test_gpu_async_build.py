@@ -120,3 +120,33 @@ def test_build_and_match_replay_as_one_cuda_graph(P):
                                        parity.make_sep_of(c, B))
         assert len(rep["borderline"]) <= 2 and rep["n_gpu"] >= na * 0.9
     assert P.hlc2_index_status(ia)[0] == P.HLC2_OK
+
+
+def test_async_like_index_against_an_index_on_another_grid(P):
+    """An index built asynchronously on C's grid, matched with B whose grid is its own (the two-grid kernel): the
+    declination extent of the asynchronous index is the whole sphere, so the tiles of its first and last zone plan their
+    windows over every B zone beyond the grid -- slower, and the pairs must still be the oracle's.  B reaches far beyond
+    C's box on both sides."""
+    rng = np.random.default_rng(73)
+    rb, db = S.uniform_patch(rng, 200_000, 80.0, 84.0, -3.0, 3.0)
+    B = S.Catalogue(rb, db, np.arange(len(rb), dtype=np.int64) * 5 + 2 * 10**12)
+    inside = (rb > 81.0) & (rb < 83.0) & (db > -0.5) & (db < 0.5)
+    k = np.flatnonzero(inside)
+    pr, pd = S.perturb(rng, B.ra[k], B.dec[k], 1.0)
+    keep = (pr > 81.0) & (pr < 83.0) & (pd > -0.5) & (pd < 0.5)
+    A = S.Catalogue(pr[keep], pd[keep], np.arange(int(keep.sum()), dtype=np.int64) * 3 + 10**12)
+    rc, dc = S.uniform_patch(rng, 30_000, 81.0, 83.0, -0.5, 0.5)
+    C = S.Catalogue(rc, dc, np.arange(len(rc), dtype=np.int64))
+    r = 2.0
+    ib = P.hlc2_build_index(*dev(B), opts=P.make_opts(r))
+    ic = P.hlc2_build_index(*dev(C), opts=P.make_opts(r, target_occupancy=0.6))
+    ia = P.hlc2_build_index(*dev(A), opts=P.make_opts(r, async_like=True), like=ic)
+    assert P.hlc2_index_status(ia) == (P.HLC2_OK, -1)
+    assert P.hlc2_grid_describe(ia)["n_cells"] != P.hlc2_grid_describe(ib)["n_cells"]
+    sep_of = parity.make_sep_of(A, B)
+    for mode in (0, 1):
+        got = P.crossmatch(ia, ib, r, mode)
+        oa, ob, os_, _ = oracle.match(A.ra, A.dec, A.id, B.ra, B.dec, B.id, r, mode)
+        cmp = parity.compare_nearest if mode else parity.compare_all_pairs
+        rep = cmp(tuple(t.cpu().numpy() for t in got), (oa, ob, os_), r, sep_of)
+        assert len(rep["borderline"]) <= 2 and rep["n_gpu"] > 0.8 * len(A)
