@@ -273,6 +273,13 @@ k_digit_scan(const uint32_t* __restrict__ digit_hist, uint32_t* __restrict__ dig
 constexpr int kOsThreads = HLC2_OS_THREADS;     // thread t owns digits t * kOsDig .. in the tile-level scans
 constexpr int kOsDig = kRadix / kOsThreads;
 constexpr int kOsCtas = 1024 / kOsThreads;      // CTAs per SM the kernel is sized for
+#ifndef HLC2_OS_LOOK
+#define HLC2_OS_LOOK 4
+#endif
+constexpr int kLook = HLC2_OS_LOOK;       // predecessor records read per look-back step
+#ifndef HLC2_OS_PREFETCH
+#define HLC2_OS_PREFETCH 1
+#endif
 #ifndef HLC2_OS_ITEMS
 #define HLC2_OS_ITEMS 18
 #endif
@@ -330,6 +337,10 @@ k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
     for (int r = 0; r < kOsItems; ++r) {
         const uint32_t t = t0 + r * 32;
         k[r] = t < cnt ? __ldg(tkeys + t) : 0xFFFFFFFFu;
+#if HLC2_OS_PREFETCH
+        // the rows are read after the ranking (three groups, each a DRAM latency if cold): ask L2 for their lines now
+        if (!FirstPass && lane == 0 && t < cnt) asm volatile("prefetch.global.L2 [%0];" :: "l"(vals + tile_base + t));
+#endif
     }
     const unsigned lt = (1u << lane) - 1;
     uint32_t* mywh = wh + w * kRadix;
@@ -338,7 +349,7 @@ k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
     // No MATCH.ANY: it measures 48 cycles per warp instruction per SM on sm_100a and alone was half of this kernel's time
     // (profiles/r2_build_experiments.md); nine ballots (one per digit bit) measure 20, the owner tags below about half of that.
 #ifndef HLC2_OS_GROUP
-#define HLC2_OS_GROUP 2
+#define HLC2_OS_GROUP 3
 #endif
     constexpr int kG = HLC2_OS_GROUP;
     static_assert(kOsItems % kG == 0, "items are ranked in groups");
@@ -435,17 +446,17 @@ k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
 #pragma unroll
     for (int q = 0; q < kOsDig; ++q) excl[q] = 0;
     if (tile > 0) {
-        // look back over the predecessors' records, eight at a time (independent loads: one memory latency per eight
+        // look back over the predecessors' records, kLook at a time (independent loads: one memory latency per kLook
         // tiles instead of one per tile); stop at the first inclusive prefix, re-poll from the first record not yet there
         long long at[kOsDig]; bool done[kOsDig]; bool all = false;
 #pragma unroll
         for (int q = 0; q < kOsDig; ++q) { at[q] = (long long)tile - 1; done[q] = false; }
         while (!all) {
-            uint32_t sv[kOsDig][8];
+            uint32_t sv[kOsDig][kLook];
 #pragma unroll
             for (int q = 0; q < kOsDig; ++q)
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
+                for (int j = 0; j < kLook; ++j) {
                     sv[q][j] = 2u << 30;                             // before tile 0: an empty inclusive prefix
                     if (!done[q] && at[q] - j >= 0) sv[q][j] = status[(size_t)(at[q] - j) * kRadix + dgt0 + q];
                 }
@@ -453,10 +464,10 @@ k_onesweep(const uint32_t* __restrict__ keys, const uint32_t* __restrict__ vals,
 #pragma unroll
             for (int q = 0; q < kOsDig; ++q) {
                 if (done[q]) continue;
-                int used = 8;
+                int used = kLook;
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    if (done[q] || used != 8) continue;
+                for (int j = 0; j < kLook; ++j) {
+                    if (done[q] || used != kLook) continue;
                     if ((sv[q][j] & kFlagMask) == 0) { used = j; continue; }
                     excl[q] += sv[q][j] & ~kFlagMask;
                     if (sv[q][j] & kFlagIncl) done[q] = true;
