@@ -567,14 +567,14 @@ void launch_gather(const Rec* rec, const uint32_t* perm, uint32_t n, double* x, 
 // the end) closes every cell above key[n-1].  Short runs are written by the owning lane, medium runs by its
 // warp, long runs (empty sky) go to a list that k_cell_fill_big spreads over the whole grid.
 // ------------------------------------------------------------------------------------------
-constexpr uint32_t kFillLane = 4, kFillWarp = 4096;
+constexpr uint32_t kFillLane = 4, kFillWarp = 4096, kFillBuf = 1024;
 
 __global__ void __launch_bounds__(256)
 k_cell_fill(const uint32_t* __restrict__ keys, uint32_t kmask, uint32_t n, uint32_t n_cells, uint32_t* __restrict__ cell_start,
             uint32_t* __restrict__ big, uint32_t* __restrict__ big_count, uint32_t big_cap) {
-    __shared__ uint32_t s_keys[8][128];
+    __shared__ uint32_t s_cells[8][kFillBuf];
     const int lane = threadIdx.x & 31;
-    uint32_t* sk = s_keys[threadIdx.x >> 5];
+    uint32_t* sc = s_cells[threadIdx.x >> 5];
     const size_t total = (size_t)n + 1;
     // a warp takes 128 consecutive rows per step, four per lane (one 16-byte load): a pass that moves 4 bytes per
     // row needs that many bytes in flight to cover the DRAM latency
@@ -591,29 +591,28 @@ k_cell_fill(const uint32_t* __restrict__ keys, uint32_t kmask, uint32_t n, uint3
         }
         uint32_t prev = __shfl_up_sync(0xffffffffu, k[3], 1);
         if (lane == 0) prev = b > 0 ? (__ldg(keys + b - 1) & kmask) : 0u;
-        // common case, no long empty run inside the 128 rows: lanes own CELLS, not rows -- cell c gets the first row of
-        // the step whose key is >= c (a binary search over the step's keys in shared memory), so the stores of a warp
-        // are consecutive words instead of scattered ones
+        // common case, the 128 rows span fewer than kFillBuf cells: every row writes its number under the cells it opens
+        // (those above the previous row's key up to its own) into a table of the warp's own in shared memory, then the
+        // warp copies the table out -- consecutive words instead of scattered ones, and no chain of dependent look-ups
         {
-            uint32_t p = prev;
-            bool longrun = false;
-#pragma unroll
-            for (int j = 0; j < 4; ++j) { longrun |= k[j] - p > kFillWarp && i0 + j < total && (i0 + j > 0); p = k[j]; }
-            if (!__any_sync(0xffffffffu, longrun)) {
-                const uint32_t lo_cell = b > 0 ? __shfl_sync(0xffffffffu, prev, 0) + 1u : 0u;
-                const uint32_t hi_cell = __shfl_sync(0xffffffffu, k[3], 31);
+            const uint32_t lo_cell = b > 0 ? __shfl_sync(0xffffffffu, prev, 0) + 1u : 0u;
+            const uint32_t hi_cell = __shfl_sync(0xffffffffu, k[3], 31);
+            if (hi_cell - lo_cell < kFillBuf || hi_cell < lo_cell) {     // hi < lo: all 128 rows lie in the previous row's cell
                 __syncwarp();
-                sk[4 * lane] = k[0]; sk[4 * lane + 1] = k[1]; sk[4 * lane + 2] = k[2]; sk[4 * lane + 3] = k[3];
-                __syncwarp();
-                if (hi_cell >= lo_cell && hi_cell - lo_cell <= 32u * kFillWarp) {
-                    for (uint64_t c = (uint64_t)lo_cell + lane; c <= hi_cell; c += 32) {
-                        uint32_t pos = 0;
+                uint32_t p = prev;
 #pragma unroll
-                        for (int st = 64; st >= 1; st >>= 1) if (sk[pos + st - 1] < (uint32_t)c) pos += st;
-                        cell_start[c] = (uint32_t)(b + pos);
+                for (int j = 0; j < 4; ++j) {
+                    const size_t i = i0 + j;
+                    if (i < total) {
+                        const uint32_t first = i > 0 ? p + 1u : 0u;
+                        for (uint32_t c = first; c <= k[j] && c >= first; ++c) sc[c - lo_cell] = (uint32_t)i;
                     }
-                    continue;
+                    p = k[j];
                 }
+                __syncwarp();
+                if (hi_cell >= lo_cell)
+                    for (uint32_t c = lane; c <= hi_cell - lo_cell; c += 32) cell_start[(size_t)lo_cell + c] = sc[c];
+                continue;
             }
         }
 #pragma unroll
@@ -715,27 +714,56 @@ k_tile_desc(const uint32_t* __restrict__ tile_first, uint32_t n_zones, const uin
             TileDesc* __restrict__ tiles) {
     const uint32_t nt = __ldg(tile_first + n_zones);
     const int lane = threadIdx.x & 31;
-    for (uint32_t t = blockIdx.x * 8 + (threadIdx.x >> 5); t < nt; t += gridDim.x * 8) {
-        uint32_t lo = 0, hi = n_zones;                // largest z with tile_first[z] <= t
-        while (hi - lo > 1) { uint32_t mid = (lo + hi) >> 1; if (__ldg(tile_first + mid) <= t) lo = mid; else hi = mid; }
-        const uint32_t z = lo, cb = __ldg(cell_base + z);
-        const uint32_t zs = __ldg(cell_start + cb), ze = __ldg(cell_start + __ldg(cell_base + z + 1));
-        const uint32_t s0 = zs + (t - __ldg(tile_first + z)) * kTile;
-        const uint32_t m = min((uint32_t)kTile, ze - s0);
-        uint32_t fl = 0;
-        for (uint32_t i = lane; i < m; i += 32) {
-            const uint32_t f = __ldg(keys + s0 + i) & ~kmask;
-            fl |= (f & kKeyGeneral) == kKeyGeneral ? kTileGeneral : ((f & kKeyDecLo ? kTileDecLo : 0u) | (f & kKeyDecHi ? kTileDecHi : 0u));
+    // kTd tiles per warp and step, their look-up chains (zone search -> cell_base -> cell_start -> keys) side by side:
+    // one chain is a dozen dependent memory latencies, and a warp with a single one in flight mostly waits
+    constexpr int kTd = 4;
+    int iters = 1; while ((1u << iters) < n_zones + 1u) ++iters;
+    for (uint32_t t0 = (blockIdx.x * 8 + (threadIdx.x >> 5)) * kTd; t0 < nt; t0 += gridDim.x * 8 * kTd) {
+        uint32_t lo[kTd], hi[kTd];
+#pragma unroll
+        for (int q = 0; q < kTd; ++q) { lo[q] = 0; hi[q] = n_zones; }          // largest z with tile_first[z] <= t
+        for (int it = 0; it < iters; ++it) {
+#pragma unroll
+            for (int q = 0; q < kTd; ++q) {
+                if (hi[q] - lo[q] > 1) { const uint32_t mid = (lo[q] + hi[q]) >> 1; if (__ldg(tile_first + mid) <= min(t0 + q, nt - 1)) lo[q] = mid; else hi[q] = mid; }
+            }
         }
-        fl = __reduce_or_sync(0xffffffffu, fl);
-        if (lane == 0) {
-            TileDesc d;
-            d.first = s0; d.count = m; d.zone = z;
-            d.k_first = (__ldg(keys + s0) & kmask) - cb; d.k_last = (__ldg(keys + s0 + m - 1) & kmask) - cb;
-            d.flags = fl; d.cb = cb;
-            d.n = __ldg(n_ra + z); d.n_lo = z > 0 ? __ldg(n_ra + z - 1) : 0u; d.n_hi = z + 1 < n_zones ? __ldg(n_ra + z + 1) : 0u;
-            d.inv_n = 1.0 / (double)d.n;
-            tiles[t] = d;
+        uint32_t cb[kTd], cbn[kTd], tf[kTd], zs[kTd], ze[kTd], s0[kTd], m[kTd], fl[kTd];
+#pragma unroll
+        for (int q = 0; q < kTd; ++q) { cb[q] = __ldg(cell_base + lo[q]); cbn[q] = __ldg(cell_base + lo[q] + 1); tf[q] = __ldg(tile_first + lo[q]); }
+#pragma unroll
+        for (int q = 0; q < kTd; ++q) { zs[q] = __ldg(cell_start + cb[q]); ze[q] = __ldg(cell_start + cbn[q]); }
+        uint32_t kv[kTd][kTile / 32];
+#pragma unroll
+        for (int q = 0; q < kTd; ++q) {
+            const uint32_t t = min(t0 + q, nt - 1);
+            s0[q] = zs[q] + (t - tf[q]) * kTile;
+            m[q] = min((uint32_t)kTile, ze[q] - s0[q]);
+#pragma unroll
+            for (int r = 0; r < kTile / 32; ++r) kv[q][r] = lane + 32 * r < m[q] ? __ldg(keys + s0[q] + lane + 32 * r) : 0u;
+        }
+#pragma unroll
+        for (int q = 0; q < kTd; ++q) {
+            uint32_t f_or = 0;
+#pragma unroll
+            for (int r = 0; r < kTile / 32; ++r) {
+                const uint32_t f = kv[q][r] & ~kmask;
+                f_or |= (f & kKeyGeneral) == kKeyGeneral ? kTileGeneral : ((f & kKeyDecLo ? kTileDecLo : 0u) | (f & kKeyDecHi ? kTileDecHi : 0u));
+            }
+            fl[q] = __reduce_or_sync(0xffffffffu, f_or);
+        }
+#pragma unroll
+        for (int q = 0; q < kTd; ++q) {
+            if (lane == q && t0 + q < nt) {                     // lane q writes tile q's descriptor
+                const uint32_t z = lo[q];
+                TileDesc d;
+                d.first = s0[q]; d.count = m[q]; d.zone = z;
+                d.k_first = (__ldg(keys + s0[q]) & kmask) - cb[q]; d.k_last = (__ldg(keys + s0[q] + m[q] - 1) & kmask) - cb[q];
+                d.flags = fl[q]; d.cb = cb[q];
+                d.n = __ldg(n_ra + z); d.n_lo = z > 0 ? __ldg(n_ra + z - 1) : 0u; d.n_hi = z + 1 < n_zones ? __ldg(n_ra + z + 1) : 0u;
+                d.inv_n = 1.0 / (double)d.n;
+                tiles[t0 + q] = d;
+            }
         }
     }
 }
@@ -746,7 +774,7 @@ void launch_tiles(const uint32_t* cell_start, const uint32_t* cell_base, const i
 #ifndef HLC2_TILE_CTAS
 #define HLC2_TILE_CTAS 64
 #endif
-    int blocks = (int)std::min<size_t>(((size_t)tile_cap + 7) / 8, (size_t)sm_count() * HLC2_TILE_CTAS);
+    int blocks = (int)std::min<size_t>(((size_t)tile_cap + 31) / 32, (size_t)sm_count() * HLC2_TILE_CTAS);
     k_tile_desc<<<std::max(blocks, 1), 256, 0, s>>>(d_tile_first, n_zones, cell_start, cell_base, reinterpret_cast<const uint32_t*>(n_ra), sorted_keys, key_mask, tiles); count_launch();
 }
 
