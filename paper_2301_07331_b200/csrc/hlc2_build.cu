@@ -1,13 +1,13 @@
 // hlc2_build.cu -- index-build kernels (NS (a)).
 //
 //   k_stats        (a1) validity, dec extent, coarse RA occupancy            16 B/source read
-//   k_keys_pack    (a1) cell key + unit vector; packs a 32-byte AoS record {x,y,z,id} in input order and
+//   k_keys_pack    (a1) cell key + window flags; packs a 32-byte AoS record {ra, dec, -, id} in input order and
 //                       accumulates the digit histograms of every radix pass  24 B read, 36 B written
 //   k_digit_scan   (a2) exclusive scan of the per-pass digit histograms (one CTA)
 //   k_onesweep     (a2) one LSD radix pass over (key, row): chained-scan ("decoupled look-back") of tile digit
 //                       counts, ranks by warp match, smem reorder so that every digit run is written
 //                       coalesced                                              8 B read, 8 B written per pass
-//   k_gather       (a3) one 32-byte sector per source (the packed record) -> cell-sorted SoA x,y,z,id
+//   k_gather       (a3) one 32-byte sector per source (the packed record) -> unit vector -> cell-sorted SoA x,y,z,id
 //   k_cell_fill    (a4) run boundaries of the sorted keys -> cell_start[] (also for empty cells), long empty
 //                       runs handed to k_cell_fill_big
 //   k_zone_tiles, k_tile_desc (a4) tile descriptors: runs of <= kTile consecutive sources inside one zone
@@ -141,13 +141,13 @@ constexpr int kKeyThreads = 256;
 // this one has a declination in [dec - r, dec + r] and an RA within asin(sin r / cos dec) of it, and zone_of / cell_of_u
 // are monotone, so its zone and cell lie between those of the window's ends evaluated with the SAME expressions that
 // file sources: flags computed from the padded window are a superset of what any query radius <= r_max needs.
-__device__ __forceinline__ uint32_t window_flags(const GridView& g, double dec, double cd, double u, int z, int nra, int k,
+__device__ __forceinline__ uint32_t window_flags(const GridView& g, double dec, float cd_lo, double u, int z, int nra, int k,
                                                  double rpad_deg, double sin_r) {
     const int zl = zone_of(g, dec - rpad_deg), zh = zone_of(g, dec + rpad_deg);
     if (zl < z - 1 || zh > z + 1) return kKeyGeneral;
     // sin of the RA half-window, in fp32 rounded up (conversions and the approximate division stay below 1e-6 relative;
     // flags only have to be a superset): an fp64 division costs as much as one of this kernel's sincos
-    const float sf = __fdividef((float)sin_r, (float)cd) * 1.000002f;    // cd = 0 (a pole): inf, the general path
+    const float sf = __fdividef((float)sin_r, cd_lo) * 1.000002f;        // cd_lo = 0 (near a pole): inf, the general path
     if (!(sf < 0.2f)) return kKeyGeneral;                             // polar rows: wide windows, rings
     const double s = (double)sf;
     const double w = fma(0.2 * s * s, s, s) * kTrig[3] + 1e-9;         // asin(s) <= s + s^3 / 5 below 0.2
@@ -179,29 +179,35 @@ k_keys_pack(const double* __restrict__ ra, const double* __restrict__ dec, const
         const long long v = v_next;
         if (i + step < n) { a_next = __ldg(ra + i + step); d_next = __ldg(dec + i + step); v_next = id ? (long long)__ldg(id + i + step) : (long long)(i + step); }
         uint32_t key = 0, flags = 0;
-        // bad coordinate: NaN components, so that no chord test against anything (another bad row, the match's
-        // sentinel slot) can pass; such rows are filed under cell 0 and never appear in a result
-        double ux = __longlong_as_double(0x7ff8000000000000ll), uy = ux, uz = ux;
+        // bad coordinate: the record carries NaNs, which the gather turns into a NaN unit vector, so that no chord test
+        // against anything (another bad row, the match's sentinel slot) can pass; such rows are filed under cell 0 and
+        // never appear in a result
+        double an = __longlong_as_double(0x7ff8000000000000ll), dd = an;
         if (coord_ok(a, d)) {
-            double an = norm_ra(a);
+            an = norm_ra(a); dd = d;
             int z = zone_of(g, d);
             int nra = __ldg(g.n_ra + z);
             const double u = box_u(g, an);
             const int k = cell_of_u(g, u, nra);
             key = __ldg(g.cell_base + z) + (uint32_t)k;
-            const double cd = unit_vector(an, d, ux, uy, uz);
             if (st) {
                 const unsigned long long b = f64_order_bits(d);
                 dmin = min(dmin, b); dmax = max(dmax, b);
                 if (u > g.span) ++nout;
             }
-            if (flagged) flags = window_flags(g, d, cd, u, z, nra, k, rpad_deg, sin_r);
+            if (flagged) {
+                // cos(dec) from below in fp32 (|error| of the conversion and of __cosf < 1e-6): the flags only have to be a
+                // superset; the unit vector itself (fp64) is computed by the gather, which waits on DRAM and has the issue
+                // slots this pass lacks
+                const float cd_lo = fmaxf(__cosf((float)d * 0.017453292f) - 1.5e-6f, 0.0f);
+                flags = window_flags(g, d, cd_lo, u, z, nra, k, rpad_deg, sin_r);
+            }
         }
         else if (st) { ++nbad; bad_row = min(bad_row, (unsigned long long)i); }
         keys[i] = key | flags;          // the sort looks at the key bits only; the flags ride along
         double2* o = reinterpret_cast<double2*>(rec + i);
-        o[0] = make_double2(ux, uy);
-        o[1] = make_double2(uz, __longlong_as_double(v));
+        o[0] = make_double2(an, dd);
+        o[1] = make_double2(0.0, __longlong_as_double(v));
         for (int p = 0; p < passes; ++p) atomicAdd(&hist[p * kRadix + ((key >> (p * kRadixBits)) & (kRadix - 1))], 1u);
     }
     __syncthreads();
@@ -528,17 +534,6 @@ int launch_radix_sort(uint32_t* keys_a, uint32_t* keys_b, uint32_t* val_a, uint3
 // ------------------------------------------------------------------------------------------
 // (a3) gather: sorted row order -> SoA unit vectors + ids.  One 32-byte sector per source.
 // ------------------------------------------------------------------------------------------
-__device__ __forceinline__ float2 pos_estimate(double x, double y, double z) {
-    // fp32 (ra, dec) estimate of the sorted row: the two-grid match locates its search window from it (padded by the
-    // error bound of exactly this chain); this kernel waits on scattered lines, so the two atan2f
-    // are free here and are paid once per build, not per match
-    const float fx = (float)x, fy = (float)y, fz = (float)z;
-    const float rxy = sqrtf(fx * fx + fy * fy);
-    float ra_f = atan2f(fy, fx) * 57.29577951f;
-    if (ra_f < 0.0f) ra_f += 360.0f;
-    return make_float2(ra_f, atan2f(fz, rxy) * 57.29577951f);
-}
-
 // A random 32-byte record costs a whole 128-byte line of DRAM traffic on this part whatever its neighbours do
 // (profiles/r2_build_experiments.md): the kernel is bound by line fetches in flight.  One row per thread and a grid far
 // larger than what is resident measured best (2.9 ms per 1e8 rows; 16 persistent CTAs per SM: 3.5 ms, their last
@@ -549,9 +544,13 @@ k_gather(const Rec* __restrict__ rec, const uint32_t* __restrict__ perm, uint32_
          float2* __restrict__ pos) {
     for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < n; i += (size_t)gridDim.x * 256) {
         const double2* q = reinterpret_cast<const double2*>(rec + __ldg(perm + i));
-        const double2 a = __ldg(q), b = __ldg(q + 1);
-        x[i] = a.x; y[i] = a.y; z[i] = b.x; out_id[i] = __double_as_longlong(b.y);
-        pos[i] = pos_estimate(a.x, a.y, b.x);
+        const double2 a = __ldg(q), b = __ldg(q + 1);          // (ra in [0, 360), dec), (-, id); NaNs mark a bad row
+        double ux = a.x, uy = a.x, uz = a.x;
+        if (a.x == a.x) unit_vector(a.x, a.y, ux, uy, uz);
+        x[i] = ux; y[i] = uy; z[i] = uz; out_id[i] = __double_as_longlong(b.y);
+        // fp32 (ra, dec) of the sorted row: the two-grid match locates its search window from it, padded by far more
+        // (kEpsRaDeg, kEpsDecDeg) than the rounding to fp32
+        pos[i] = make_float2((float)a.x, (float)a.y);
     }
 }
 

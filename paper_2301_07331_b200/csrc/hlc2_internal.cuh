@@ -75,7 +75,7 @@ struct IndexView {
 };
 
 // packed per-source record in INPUT order, written by the key pass and read (one sector) by the gather
-struct __align__(32) Rec { double x, y, z; long long id; };
+struct __align__(32) Rec { double ra, dec, spare; long long id; };     // ra normalised to [0, 360); NaNs: bad row
 
 // extent statistics written by the stats pass
 struct Stats {
