@@ -5,14 +5,14 @@
 //                       accumulates the digit histograms of every radix pass  24 B read, 36 B written
 //   k_digit_scan   (a2) exclusive scan of the per-pass digit histograms (one CTA)
 //   k_onesweep     (a2) one LSD radix pass over (key, row): chained-scan ("decoupled look-back") of tile digit
-//                       counts, ranks by warp match, smem reorder so that every digit run is written
+//                       counts, ranks by owner tags and votes, smem reorder so that every digit run is written
 //                       coalesced                                              8 B read, 8 B written per pass
 //   k_gather       (a3) one 32-byte sector per source (the packed record) -> unit vector -> cell-sorted SoA x,y,z,id
 //   k_cell_fill    (a4) run boundaries of the sorted keys -> cell_start[] (also for empty cells), long empty
 //                       runs handed to k_cell_fill_big
 //   k_zone_tiles, k_tile_desc (a4) tile descriptors: runs of <= kTile consecutive sources inside one zone
 //
-// All of them are HBM-bound streaming passes; grids are multiples of the SM count.
+// All of them are streaming passes; persistent grids are multiples of the SM count, the gather runs one row per thread.
 #include <string.h>
 #include <algorithm>
 
