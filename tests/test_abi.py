@@ -63,6 +63,7 @@ def test_null_handles_are_rejected(P):
     assert L.hlc2_index_status(None, None) == P.HLC2_ERR_INVALID_ARG
     assert L.hlc2_grid_describe(None, None, None) == P.HLC2_ERR_INVALID_ARG
     assert L.hlc2_crossmatch(None, None, 1.0, 0, None, None, None, 0, None, None, 0, None) == P.HLC2_ERR_INVALID_ARG
+    assert L.hlc2_crossmatch_static(None, None, 1.0, 0, None, None, None, 0, None, None) == P.HLC2_ERR_INVALID_ARG
     out = ctypes.c_void_p()
     assert L.hlc2_build_index(None, None, None, 5, None, None, 0, None, 0, None, ctypes.byref(out)) == P.HLC2_ERR_INVALID_ARG
     L.hlc2_index_destroy(None)
@@ -71,11 +72,12 @@ def test_null_handles_are_rejected(P):
 def test_error_strings(P):
     L = P.lib()
     seen = set()
-    for code in range(0, -8, -1):
+    for code in range(0, -9, -1):
         s = L.hlc2_strerror(code).decode()
         assert s and s != "unknown status"
         seen.add(s)
-    assert len(seen) == 8
+    assert len(seen) == 9
+    assert "8 MiB" in L.hlc2_strerror(P.HLC2_ERR_STATIC_LIMIT).decode()          # the limit is named in the message
     assert L.hlc2_strerror(-99).decode() == "unknown status"
     assert "sm_100a" in P.version()
 
